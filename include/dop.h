@@ -1,0 +1,145 @@
+/*
+ * dop.h -- C-ABI boundary of the B200-native angular-spectrum (ASM) propagation library.
+ *
+ * One data-parallel hot path: scalar ASM free-space propagation of a DOE height map on very
+ * large grids (forward), and its adjoint (dL/dI -> dL/dh).  Citations are to
+ * /root/reference/PAPER.md (arxiv 2505.22313), section 3.1:
+ *
+ *   Eq. (1) PAPER.md:95-99    Phi_lambda(x,y) = (2 pi / lambda) (n_lambda - 1) h(x,y)
+ *   Eq. (2) PAPER.md:99-102   E_doe = E_in * exp(i Phi)                  (E_in == 1 here)
+ *   Eq. (3) PAPER.md:104-108  E_dest = F^-1{ F{E_doe} (x) H_lambda }     (F = 2-D FFT)
+ *   Eq. (4) PAPER.md:108-112  I_lambda = |E_dest|^2, objective sum_lambda L_p(I_lambda)
+ *   back-propagation: PAPER.md:124; "backward pass is realized by another ... 2-D FFT"
+ *   PAPER.md:200 (section 4.1); row-column decomposition of the 2-D FFT PAPER.md:200.
+ *
+ * Readings where the paper is silent ("Readings"):
+ *   H_lambda[ky,kx] = exp(+i 2 pi z sqrt(a)) if a >= 0 else 0,
+ *       a = (1/lambda^2 - fx^2) - fy^2, fx = kx/(nx pitch), fy = ky/(ny pitch), signed bins
+ *       (BASELINE.json north_star; the paper never writes H out);
+ *   forward DFT kernel exp(-2 pi i k n/N) unnormalised, inverse exp(+...) scaled 1/(ny nx);
+ *   loss (DOP_LOSS_L2) L = sum_lambda (1/(ny nx)) sum_{y,x} (I_lambda - T)^2;
+ *   pre-filter (sigma > 0): h <- Re F^-1{ F{h} exp(-2 pi^2 sigma^2 ((kx/nx)^2+(ky/ny)^2)) }.
+ *
+ * Conventions
+ *   Layout     every plane is row-major [ny][nx], x contiguous; [n_lambda][ny][nx] where noted.
+ *   Pointers   "host" or "device" is stated per argument.  The caller owns every device buffer
+ *              including the workspace; the plan owns host memory and small device tables
+ *              (O(nx + ny) bytes, allocated on the current device at the first propagate call,
+ *              freed by dop_plan_destroy).  The library never allocates O(ny nx) memory.
+ *   Alignment  device planes must be 16-byte aligned (any cudaMalloc / torch allocation is).
+ *   Asynchrony dop_propagate_* only enqueue kernels on `cuda_stream` (a cudaStream_t passed as
+ *              void*; NULL = the legacy default stream) and never synchronise it.
+ *   State      between dop_propagate_fwd and dop_propagate_adj the workspace holds the
+ *              destination field (DOP_LOSS_NONE) or the seeded, partly transformed gradient
+ *              field (DOP_LOSS_L2); the caller must not touch it.  dop_propagate_adj without a
+ *              preceding successful dop_propagate_fwd on the same plan -> DOP_ERR_STATE.
+ *   Errors     every call returns a dop_status; argument / size / state errors are detected
+ *              before anything is enqueued.  No exception crosses the boundary, there is no
+ *              global state, and there is NO CPU fallback: without an sm_100 device the
+ *              propagate calls fail with DOP_ERR_ARCH / DOP_ERR_CUDA.
+ */
+#ifndef DOP_H_
+#define DOP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dop_plan dop_plan; /* opaque, host-side */
+
+typedef enum {
+    DOP_OK = 0,
+    DOP_ERR_INVALID_ARG = 1,      /* NULL where a pointer is required, non-finite / non-positive
+                                     pitch or lambda, n_lambda < 1, bad enum, missing buffer     */
+    DOP_ERR_UNSUPPORTED_SIZE = 2, /* ny or nx < 2, or not of the form 2^a 3^b                    */
+    DOP_ERR_WORKSPACE = 3,        /* NULL workspace                                              */
+    DOP_ERR_STATE = 4,            /* adj called before fwd                                       */
+    DOP_ERR_ARCH = 5,             /* current device is not compute capability 10.x (sm_100)      */
+    DOP_ERR_CUDA = 6              /* a CUDA runtime call or launch failed (cudaGetLastError)     */
+} dop_status;
+
+typedef enum {
+    DOP_LOSS_NONE = 0, /* fwd writes I (and keeps the field); adj takes the caller's dL/dI       */
+    DOP_LOSS_L2 = 1    /* L = sum_lambda mean_xy (I_lambda - T)^2, seeded inside the pass (Eq. 4) */
+} dop_loss_mode;
+
+/* flags */
+#define DOP_WRITE_INTENSITY 0x1u /* DOP_LOSS_L2 only: also write I to d_intensity                */
+
+typedef struct {
+    int64_t ny, nx;            /* rows, columns; x contiguous; each 2^a 3^b, >= 2               */
+    double pitch;              /* metres, same in x and y                                        */
+    int32_t n_lambda;          /* >= 1                                                           */
+    const double* lambda;      /* [n_lambda] metres, HOST memory, copied by dop_plan_create      */
+    const double* n_refr;      /* [n_lambda] refractive index n_lambda (Eq. 1), HOST, copied     */
+    double z;                  /* metres, any sign, 0 allowed                                    */
+    dop_loss_mode loss;
+    double prefilter_sigma_px; /* 0 = off; > 0 = Gaussian spectral pre-filter on h (config 3)    */
+    uint32_t flags;            /* DOP_WRITE_INTENSITY                                            */
+} dop_plan_desc;
+
+/*
+ * Build a plan (host-only work: validation, factorisation of ny and nx into radix-2/3/4 digit
+ * passes, twiddle / frequency tables in fp64, pass schedule).  Touches no GPU.
+ *   out              receives the plan (host pointer).
+ *   workspace_bytes  (may be NULL) receives the size of the device workspace the caller must
+ *                    pass to the propagate calls: n_lambda complex64 fields + (pre-filter on)
+ *                    one fp32 plane + loss-reduction scratch.
+ * Errors: DOP_ERR_INVALID_ARG, DOP_ERR_UNSUPPORTED_SIZE.
+ */
+dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* workspace_bytes);
+
+/*
+ * Forward pass, Eq. (1)-(4): for every lambda  h -> Phi -> u0 = exp(i Phi) -> F -> (x) H ->
+ * F^-1 -> I = |u|^2 [-> L2 loss and the seed g_u = 2 (dL/dI) u of the adjoint, DOP_LOSS_L2].
+ *   d_height     [ny][nx] fp32 DEVICE, metres, read-only.
+ *   d_target     [ny][nx] fp32 DEVICE (shared by all lambda); required for DOP_LOSS_L2,
+ *                ignored (may be NULL) for DOP_LOSS_NONE.
+ *   d_intensity  [n_lambda][ny][nx] fp32 DEVICE; required for DOP_LOSS_NONE and for
+ *                DOP_LOSS_L2 with DOP_WRITE_INTENSITY; otherwise ignored (may be NULL).
+ *   d_loss       DEVICE double scalar or NULL; DOP_LOSS_L2: receives L when the stream reaches
+ *                that point.  Ignored for DOP_LOSS_NONE.
+ *   d_workspace  DEVICE, workspace_bytes from dop_plan_create, 256-byte aligned.
+ *                After a DOP_LOSS_NONE forward its first n_lambda*ny*nx complex64 (interleaved
+ *                re, im) hold the destination field u of Eq. (3), natural order.
+ *   cuda_stream  cudaStream_t.
+ */
+dop_status dop_propagate_fwd(dop_plan* plan, const float* d_height, const float* d_target,
+                             float* d_intensity, double* d_loss, void* d_workspace,
+                             void* cuda_stream);
+
+/*
+ * Adjoint pass: dL/dI -> g_u = 2 (dL/dI) u -> F -> (x) conj(H) -> F^-1 ->
+ * dL/dh = sum_lambda (2 pi (n_lambda-1)/lambda) Im( conj(u0) g_u0 )  [-> pre-filter adjoint].
+ *   d_height       the same buffer that was given to dop_propagate_fwd (u0 is recomputed).
+ *   d_dLdI         [n_lambda][ny][nx] fp32 DEVICE; required for DOP_LOSS_NONE, ignored for
+ *                  DOP_LOSS_L2 (the seed was formed inside the forward pass).
+ *   d_grad_height  [ny][nx] fp32 DEVICE, overwritten with dL/dh.
+ */
+dop_status dop_propagate_adj(dop_plan* plan, const float* d_height, const float* d_dLdI,
+                             float* d_grad_height, void* d_workspace, void* cuda_stream);
+
+/* Frees the plan's host memory and device tables.  NULL -> DOP_ERR_INVALID_ARG. */
+dop_status dop_plan_destroy(dop_plan* plan);
+
+/* Static string for a status code (never NULL). */
+const char* dop_status_string(dop_status s);
+
+/*
+ * Introspection (host only): writes a NUL-terminated, line-oriented description of the pass
+ * schedule (one line per kernel launch of one lambda's forward+adjoint, with digit lengths,
+ * tile shapes and algorithmic HBM bytes per point) into buf[0..len).  Returns the number of
+ * bytes the full text needs (excluding the NUL); output is truncated to len-1 bytes.
+ */
+size_t dop_plan_describe(const dop_plan* plan, char* buf, size_t len);
+
+/* Number of kernel launches one dop_propagate_fwd + dop_propagate_adj pair enqueues. */
+int64_t dop_plan_launch_count(const dop_plan* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DOP_H_ */

@@ -1,0 +1,298 @@
+// api.cu -- the C-ABI entry points declared in include/dop.h: validation, lazy upload of the
+// plan's small device tables, and the enqueueing of the pass schedule.  No torch types, no
+// synchronisation, no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "dop_internal.h"
+
+namespace dop {
+cudaError_t launch_tile_pass_generic(const PassDesc& p, cudaStream_t stream);
+cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* handled);
+
+cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream)
+{
+    static const bool force_generic = std::getenv("DOP_FORCE_GENERIC") != nullptr;
+    if (!force_generic) {
+        bool handled = false;
+        cudaError_t e = launch_tile_pass_pow2(p, stream, &handled);
+        if (handled) return e;
+    }
+    return launch_tile_pass_generic(p, stream);
+}
+} // namespace dop
+
+using namespace dop;
+
+namespace {
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Buffers {
+    const float* height = nullptr; // what LD_HEIGHT / ST_GRAD read (h or h_eff)
+    const float* target = nullptr;
+    float* intensity = nullptr;
+    const float* dLdI = nullptr;
+    float* grad = nullptr;
+    const float* real_src = nullptr;
+    float* real_dst = nullptr;
+};
+
+dop_status ensure_device(dop_plan* p)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return DOP_ERR_CUDA;
+    if (p->dev_ready && p->device == dev) return DOP_OK;
+    if (p->dev_ready) return DOP_ERR_INVALID_ARG; // a plan is bound to the device of its first use
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return DOP_ERR_CUDA;
+    if (major != 10) return DOP_ERR_ARCH;
+
+    // arena layout: W_L tables | boundary twiddles | pi tables | f2 x,y | g x,y
+    size_t off = 0;
+    p->wl_off.resize(p->wl_tables.size());
+    for (size_t i = 0; i < p->wl_tables.size(); ++i) { p->wl_off[i] = off; off += align256(p->wl_tables[i].size() * sizeof(float2)); }
+    for (int a = 0; a < 2; ++a)
+        for (Digit& g : p->ax[a].dig)
+            if (g.has_twb) { g.twb_off = off; off += align256(g.twb.size() * sizeof(float2)); }
+    for (int a = 0; a < 2; ++a) {
+        p->pi_off[a].resize(p->ax[a].dig.size());
+        for (size_t j = 0; j < p->ax[a].dig.size(); ++j) { p->pi_off[a][j] = off; off += align256(p->ax[a].dig[j].pi.size() * sizeof(int)); }
+    }
+    size_t f2_off[2], g_off[2];
+    for (int a = 0; a < 2; ++a) { f2_off[a] = off; off += align256(p->ax[a].f2.size() * sizeof(double)); }
+    for (int a = 0; a < 2; ++a) { g_off[a] = off; off += align256(p->ax[a].g.size() * sizeof(float)); }
+
+    char* arena = nullptr;
+    if (cudaMalloc((void**)&arena, off) != cudaSuccess) return DOP_ERR_CUDA;
+    p->d_arena = arena;
+    bool ok = true;
+    auto up = [&](size_t o, const void* src, size_t bytes) {
+        if (bytes && cudaMemcpy(arena + o, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
+    };
+    for (size_t i = 0; i < p->wl_tables.size(); ++i) up(p->wl_off[i], p->wl_tables[i].data(), p->wl_tables[i].size() * sizeof(float2));
+    for (int a = 0; a < 2; ++a)
+        for (Digit& g : p->ax[a].dig)
+            if (g.has_twb) up(g.twb_off, g.twb.data(), g.twb.size() * sizeof(float2));
+    for (int a = 0; a < 2; ++a)
+        for (size_t j = 0; j < p->ax[a].dig.size(); ++j) up(p->pi_off[a][j], p->ax[a].dig[j].pi.data(), p->ax[a].dig[j].pi.size() * sizeof(int));
+    for (int a = 0; a < 2; ++a) {
+        up(f2_off[a], p->ax[a].f2.data(), p->ax[a].f2.size() * sizeof(double));
+        up(g_off[a], p->ax[a].g.data(), p->ax[a].g.size() * sizeof(float));
+        p->d_f2[a] = (double*)(arena + f2_off[a]);
+        p->d_g[a] = (float*)(arena + g_off[a]);
+    }
+    if (!ok) { cudaFree(arena); p->d_arena = nullptr; return DOP_ERR_CUDA; }
+    p->device = dev;
+    p->dev_ready = true;
+    return DOP_OK;
+}
+
+// Resolve one scheduled pass for wavelength `lam` into launch parameters.
+PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b, char* ws)
+{
+    PassDesc d{};
+    tile_geometry(p, t.axis, t.digit, &d);
+    const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
+    char* arena = (char*)p->d_arena;
+    const size_t npts = (size_t)p->desc.nx * (size_t)p->desc.ny;
+    d.fft1_dir = t.fft1_dir;
+    d.fft2_dir = t.fft2_dir;
+    d.wL = (const float2*)(arena + p->wl_off[(size_t)g.wl_index]);
+    d.pi = (const int*)(arena + p->pi_off[t.axis][(size_t)t.digit]);
+    d.tw_b = g.has_twb ? (const float2*)(arena + g.twb_off) : nullptr;
+    d.load_op = t.load_op;
+    d.mid_op = t.mid_op;
+    d.store_op = t.store_op;
+    d.field = (float2*)(ws + align256(npts * sizeof(float2)) * (size_t)lam);
+    d.height = b.height;
+    d.write_intensity = 0;
+    if (t.load_op == LD_SEED) d.plane_in = b.dLdI + npts * (size_t)lam;
+    if (t.load_op == LD_REAL) d.plane_in = b.real_src;
+    if (t.mid_op == MID_LOSS) {
+        d.plane_in = b.target;
+        d.loss_scratch = (double*)(ws + p->ws_loss_off) + (size_t)p->loss_tiles * (size_t)lam;
+        if (p->desc.flags & DOP_WRITE_INTENSITY) {
+            d.write_intensity = 1;
+            d.plane_out = b.intensity + npts * (size_t)lam;
+        }
+    }
+    if (t.store_op == ST_GRAD) {
+        d.plane_out = b.grad;
+        if (lam > 0) d.store_op = ST_GRAD_ACC;
+    }
+    if (t.store_op == ST_C64_INTENSITY) d.plane_out = b.intensity + npts * (size_t)lam;
+    if (t.store_op == ST_REAL) d.plane_out = b.real_dst;
+    const double lambda = p->lambda[(size_t)lam], n = p->n_refr[(size_t)lam];
+    d.phase_coef = (float)((n - 1.0) / lambda);
+    d.grad_coef = (float)(2.0 * M_PI * (n - 1.0) / lambda);
+    d.scale = (float)(1.0 / (double)npts);
+    d.seed_coef = (float)(4.0 / (double)npts);
+    d.inv_lam2 = 1.0 / (lambda * lambda);
+    d.z = p->desc.z;
+    d.fx2 = p->d_f2[0];
+    d.fy2 = p->d_f2[1];
+    d.gx = p->d_g[0];
+    d.gy = p->d_g[1];
+    return d;
+}
+
+dop_status run(const dop_plan* p, const std::vector<PassTmpl>& sched, int lam, const Buffers& b, char* ws,
+               cudaStream_t st)
+{
+    for (const PassTmpl& t : sched) {
+        PassDesc d = resolve(p, t, lam, b, ws);
+        if (launch_tile_pass(d, st) != cudaSuccess) return DOP_ERR_CUDA;
+    }
+    return DOP_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* workspace_bytes)
+{
+    if (out == nullptr) return DOP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (d == nullptr || d->lambda == nullptr || d->n_refr == nullptr) return DOP_ERR_INVALID_ARG;
+    if (d->n_lambda < 1 || d->n_lambda > 4096) return DOP_ERR_INVALID_ARG;
+    if (!(d->pitch > 0.0) || !std::isfinite(d->pitch) || !std::isfinite(d->z)) return DOP_ERR_INVALID_ARG;
+    if (!(d->prefilter_sigma_px >= 0.0) || !std::isfinite(d->prefilter_sigma_px)) return DOP_ERR_INVALID_ARG;
+    if (d->loss != DOP_LOSS_NONE && d->loss != DOP_LOSS_L2) return DOP_ERR_INVALID_ARG;
+    if (d->flags & ~DOP_WRITE_INTENSITY) return DOP_ERR_INVALID_ARG;
+    for (int i = 0; i < d->n_lambda; ++i) {
+        if (!(d->lambda[i] > 0.0) || !std::isfinite(d->lambda[i])) return DOP_ERR_INVALID_ARG;
+        if (!std::isfinite(d->n_refr[i])) return DOP_ERR_INVALID_ARG;
+    }
+    if (d->ny < 2 || d->nx < 2) return DOP_ERR_UNSUPPORTED_SIZE;
+    dop_plan* p = new (std::nothrow) dop_plan();
+    if (p == nullptr) return DOP_ERR_INVALID_ARG;
+    p->desc = *d;
+    p->lambda.assign(d->lambda, d->lambda + d->n_lambda);
+    p->n_refr.assign(d->n_refr, d->n_refr + d->n_lambda);
+    p->desc.lambda = p->lambda.data();
+    p->desc.n_refr = p->n_refr.data();
+    dop_status s;
+    try {
+        s = build_plan(p);
+    } catch (...) {
+        s = DOP_ERR_INVALID_ARG;
+    }
+    if (s != DOP_OK) { delete p; return s; }
+    if (workspace_bytes) *workspace_bytes = p->ws_bytes;
+    *out = p;
+    return DOP_OK;
+}
+
+dop_status dop_propagate_fwd(dop_plan* p, const float* d_height, const float* d_target, float* d_intensity,
+                             double* d_loss, void* d_workspace, void* cuda_stream)
+{
+    if (p == nullptr || d_height == nullptr) return DOP_ERR_INVALID_ARG;
+    const bool l2 = p->desc.loss == DOP_LOSS_L2;
+    const bool need_I = !l2 || (p->desc.flags & DOP_WRITE_INTENSITY);
+    if (l2 && d_target == nullptr) return DOP_ERR_INVALID_ARG;
+    if (need_I && d_intensity == nullptr) return DOP_ERR_INVALID_ARG;
+    if (d_workspace == nullptr) return DOP_ERR_WORKSPACE;
+    dop_status s = ensure_device(p);
+    if (s != DOP_OK) return s;
+    p->state = 0;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* ws = (char*)d_workspace;
+    Buffers b;
+    b.height = d_height;
+    b.target = d_target;
+    b.intensity = d_intensity;
+    if (!p->pre.empty()) { // F0: h_eff = Re F^-1{ F{h} G }
+        float* heff = (float*)(ws + p->ws_heff_off);
+        Buffers pb;
+        pb.real_src = d_height;
+        pb.real_dst = heff;
+        if ((s = run(p, p->pre, 0, pb, ws, st)) != DOP_OK) return s;
+        b.height = heff;
+    }
+    for (int lam = 0; lam < p->desc.n_lambda; ++lam)
+        if ((s = run(p, p->fwd, lam, b, ws, st)) != DOP_OK) return s;
+    if (l2 && d_loss != nullptr) {
+        const double inv_n = 1.0 / ((double)p->desc.nx * (double)p->desc.ny);
+        if (launch_loss_reduce((const double*)(ws + p->ws_loss_off), p->loss_tiles * p->desc.n_lambda, inv_n, d_loss,
+                               st) != cudaSuccess)
+            return DOP_ERR_CUDA;
+    }
+    p->state = 1;
+    return DOP_OK;
+}
+
+dop_status dop_propagate_adj(dop_plan* p, const float* d_height, const float* d_dLdI, float* d_grad_height,
+                             void* d_workspace, void* cuda_stream)
+{
+    if (p == nullptr || d_height == nullptr || d_grad_height == nullptr) return DOP_ERR_INVALID_ARG;
+    if (p->desc.loss == DOP_LOSS_NONE && d_dLdI == nullptr) return DOP_ERR_INVALID_ARG;
+    if (d_workspace == nullptr) return DOP_ERR_WORKSPACE;
+    if (p->state != 1) return DOP_ERR_STATE;
+    dop_status s = ensure_device(p);
+    if (s != DOP_OK) return s;
+    p->state = 0;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* ws = (char*)d_workspace;
+    Buffers b;
+    b.height = p->pre.empty() ? d_height : (const float*)(ws + p->ws_heff_off);
+    b.dLdI = d_dLdI;
+    b.grad = d_grad_height;
+    for (int lam = 0; lam < p->desc.n_lambda; ++lam)
+        if ((s = run(p, p->adj, lam, b, ws, st)) != DOP_OK) return s;
+    if (!p->pre.empty()) { // A6: the Gaussian spectrum is real and even, so the filter is self-adjoint
+        Buffers pb;
+        pb.real_src = d_grad_height;
+        pb.real_dst = d_grad_height;
+        if ((s = run(p, p->pre, 0, pb, ws, st)) != DOP_OK) return s;
+    }
+    return DOP_OK;
+}
+
+dop_status dop_plan_destroy(dop_plan* p)
+{
+    if (p == nullptr) return DOP_ERR_INVALID_ARG;
+    if (p->d_arena != nullptr) cudaFree(p->d_arena);
+    delete p;
+    return DOP_OK;
+}
+
+const char* dop_status_string(dop_status s)
+{
+    switch (s) {
+    case DOP_OK: return "DOP_OK";
+    case DOP_ERR_INVALID_ARG: return "DOP_ERR_INVALID_ARG: bad or missing argument";
+    case DOP_ERR_UNSUPPORTED_SIZE: return "DOP_ERR_UNSUPPORTED_SIZE: ny and nx must be 2^a 3^b, >= 2";
+    case DOP_ERR_WORKSPACE: return "DOP_ERR_WORKSPACE: workspace missing";
+    case DOP_ERR_STATE: return "DOP_ERR_STATE: dop_propagate_adj needs a preceding dop_propagate_fwd";
+    case DOP_ERR_ARCH: return "DOP_ERR_ARCH: device is not sm_100";
+    case DOP_ERR_CUDA: return "DOP_ERR_CUDA: CUDA runtime error (see cudaGetLastError)";
+    }
+    return "DOP_ERR_UNKNOWN";
+}
+
+size_t dop_plan_describe(const dop_plan* p, char* buf, size_t len)
+{
+    if (p == nullptr) return 0;
+    std::string s = describe_plan(p);
+    if (buf != nullptr && len > 0) {
+        size_t n = s.size() < len - 1 ? s.size() : len - 1;
+        std::memcpy(buf, s.data(), n);
+        buf[n] = '\0';
+    }
+    return s.size();
+}
+
+int64_t dop_plan_launch_count(const dop_plan* p)
+{
+    if (p == nullptr) return 0;
+    int64_t n = (int64_t)(p->fwd.size() + p->adj.size()) * p->desc.n_lambda + 2 * (int64_t)p->pre.size();
+    if (p->desc.loss == DOP_LOSS_L2) n += 1;
+    return n;
+}
+
+} // extern "C"

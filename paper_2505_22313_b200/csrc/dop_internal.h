@@ -1,0 +1,159 @@
+// dop_internal.h -- shared declarations of the CUDA path (plan <-> kernels <-> C-ABI).
+// Nothing here is shared with oracle/ (the oracle is independent test infrastructure).
+//
+// Vocabulary ("Decomposition"):
+//   axis    x (contiguous, length nx) or y (strided, length ny).
+//   digit   an axis length N is factored N = L_0 L_1 ... L_{m-1}; index n = sum n_j st_j with
+//           st_j = prod_{i>j} L_i.  One *pass* (one kernel launch, one read + one write of the
+//           field) transforms one digit of one axis: an L_j-point in-place DFT on every line
+//           {base + i*es, i < L_j}.  Forward = decimation in frequency: digits most-significant
+//           first, then the "boundary twiddle" T_j = W_{N_j}^{k_j r_j} (N_j = L_j st_j,
+//           r_j = n mod st_j).  Spectra stay in this digit-scrambled slot order; the inverse is
+//           the exact mirror (conj(T_j) first, digits least-significant first), so no reorder
+//           pass ever runs and H is evaluated at the true frequency of each slot from tables.
+//   tile    what one CTA holds on chip: nl lines x L points.
+//           column-type: the nl lines are adjacent in memory (line stride 1), elements es apart;
+//           row-type:    each line is L contiguous elements (es = 1).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include <string>
+#include <vector>
+
+#include "../../include/dop.h"
+
+namespace dop {
+
+enum LoadOp : int {
+    LD_C64 = 0,     // complex64 field
+    LD_HEIGHT = 1,  // Eq. (1)+(2): u0 = exp(i 2 pi (n-1) h / lambda) from the fp32 height plane
+    LD_SEED = 2,    // A1 (DOP_LOSS_NONE): g_u = 2 (dL/dI) u
+    LD_REAL = 3     // pre-filter: fp32 plane -> (v, 0)
+};
+enum MidOp : int {
+    MID_NONE = 0,
+    MID_H = 1,      // (x) H_lambda of Eq. (3), scaled by 1/(ny nx)
+    MID_HCONJ = 2,  // (x) conj(H_lambda) (adjoint), scaled by 1/(ny nx)
+    MID_GAUSS = 3,  // pre-filter spectrum factor, scaled by 1/(ny nx)
+    MID_LOSS = 4    // I = |u|^2, L2 loss partial, seed g_u = (4/N)(I - T) u  [optional I write]
+};
+enum StoreOp : int {
+    ST_C64 = 0,
+    ST_GRAD = 1,           // A5: dL/dh  = c Im(conj(u0) g)   (overwrite)
+    ST_GRAD_ACC = 2,       //     dL/dh += ...                (lambda > 0)
+    ST_C64_INTENSITY = 3,  // DOP_LOSS_NONE forward end: keep u, write I
+    ST_REAL = 4            // pre-filter: Re(v) -> fp32 plane
+};
+
+constexpr int kMaxRadixSteps = 16;
+
+// Everything one launch of the generic tile kernel needs (passed by value).
+struct PassDesc {
+    // ---- tile geometry
+    int L;        // digit length
+    int nl;       // lines per tile
+    int col_type; // 1 = column-type tile, 0 = row-type
+    long long es; // element stride (elements of the plane)
+    long long NC, SCc; // lines along c: count, stride
+    long long n_m, SM; // middle coordinate
+    long long n_o, SO; // outer coordinate
+    long long n_cgroups;
+    // ---- in-tile DFT
+    int n_radix;
+    int radix[kMaxRadixSteps];
+    int fft1_dir; // +1 forward (exp -), -1 inverse (exp +)
+    int fft2_dir; // 0 = none
+    const float2* wL;   // [L]  W_L^p = exp(-2 pi i p / L)
+    const int* pi;      // [L]  slot within digit -> output index k_j
+    const float2* tw_b; // [N_j] boundary twiddles W_{N_j}^p, or nullptr
+    int r_from;         // 0: r_j = c (x digit), 1: r_j = m (y digit)
+    // ---- pointwise ops
+    int load_op, mid_op, store_op;
+    int write_intensity;
+    float2* field;
+    const float* height;  // LD_HEIGHT / ST_GRAD*
+    const float* plane_in; // LD_SEED: dL/dI;  LD_REAL: source;  MID_LOSS: target T
+    float* plane_out;     // ST_GRAD*: grad;  ST_REAL: destination;  *_INTENSITY: I
+    double* loss_scratch; // MID_LOSS: one partial per CTA
+    float phase_coef;     // (n-1)/lambda   [turns per metre]
+    float grad_coef;      // 2 pi (n-1)/lambda
+    float scale;          // 1/(ny nx)
+    float seed_coef;      // 4/(ny nx)
+    double inv_lam2, z;   // H
+    const double* fx2;    // [nx] slot -> fx^2   (fp64, same expression as the definition)
+    const double* fy2;    // [ny] slot -> fy^2
+    const float* gx;      // [nx] slot -> Gaussian factor
+    const float* gy;      // [ny]
+    long long row_o, row_m, row_i; // y slot of element i: o*row_o + m*row_m + i*row_i
+    int smem_bytes;
+    int threads;
+};
+
+cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream);
+cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
+                               cudaStream_t stream);
+
+// ------------------------------------------------------------------------------------------
+// host-side plan
+// ------------------------------------------------------------------------------------------
+struct Digit {
+    long long L = 0, st = 0;      // length, slot stride within the axis
+    std::vector<int> radix;       // in-place DIF radix steps, product = L
+    std::vector<int> pi;          // slot -> k_j
+    int wl_index = -1;            // which W_L table
+    bool has_twb = false;
+    std::vector<float2> twb;      // W_{L st}^p, p < L st
+    size_t twb_off = 0;           // offset (float2) into the device twiddle arena
+};
+
+struct Axis {
+    long long N = 0;
+    std::vector<Digit> dig;
+    std::vector<long long> kslot; // slot -> frequency index in [0, N)
+    std::vector<double> f2;       // slot -> f^2
+    std::vector<float> g;         // slot -> Gaussian factor (pre-filter)
+};
+
+enum Buf : int { BUF_NONE = 0, BUF_HEIGHT, BUF_HEFF, BUF_TARGET, BUF_INTENSITY, BUF_DLDI, BUF_GRAD };
+
+// A pass with symbolic buffers; resolved to a PassDesc at launch time.
+struct PassTmpl {
+    int axis;  // 0 = x, 1 = y
+    int digit;
+    int fft1_dir, fft2_dir;
+    int load_op, mid_op, store_op;
+    std::string name;
+    double bytes_per_point; // algorithmic HBM bytes per grid point of this launch
+};
+
+} // namespace dop
+
+struct dop_plan {
+    dop_plan_desc desc;
+    std::vector<double> lambda, n_refr;
+    dop::Axis ax[2]; // 0 = x, 1 = y
+    std::vector<std::vector<float2>> wl_tables; // distinct W_L tables
+    std::vector<long long> wl_len;
+    std::vector<size_t> wl_off;
+    int tile_pts = 4096;
+    // schedules for one lambda
+    std::vector<dop::PassTmpl> fwd, adj, pre; // pre = Gaussian pre-filter (real -> real)
+    long long loss_tiles = 0;                 // CTAs of the MID_LOSS pass
+    size_t ws_fields = 0, ws_heff_off = 0, ws_loss_off = 0, ws_bytes = 0;
+    // device tables (lazy)
+    bool dev_ready = false;
+    int device = -1;
+    void* d_arena = nullptr;
+    float2* d_tw = nullptr; // W_L tables then boundary twiddles
+    int* d_pi = nullptr;
+    double* d_f2[2] = {nullptr, nullptr};
+    float* d_g[2] = {nullptr, nullptr};
+    std::vector<size_t> pi_off[2];
+    int state = 0; // 1 after a successful fwd
+};
+
+namespace dop {
+dop_status build_plan(dop_plan* p);
+std::string describe_plan(const dop_plan* p);
+void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d);
+} // namespace dop

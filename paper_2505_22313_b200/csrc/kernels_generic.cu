@@ -1,0 +1,290 @@
+// kernels_generic.cu -- the generic tile-pass kernel: any digit length 2^a 3^b, any tile shape,
+// every fused pointwise op.  One CTA = one tile held in shared memory; in-place mixed-radix
+// (2/3/4) decimation-in-frequency forward, mirrored decimation-in-time inverse.
+// It is the correctness backbone and the fallback for shapes the specialised kernels
+// (kernels_pow2.cu) do not cover.
+//
+// Math (Eq. 1-4; PAPER.md:200 row-column 2-D FFT):
+//   forward digit pass : v <- DFT_L(v) along the line, then v *= T_j      (T_j boundary twiddle)
+//   inverse digit pass : v *= conj(T_j), then v <- L * IDFT_L(v)          (1/N folded into H)
+#include "dop_internal.h"
+
+namespace dop {
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) // a * conj(b)
+{
+    return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+
+// one radix-r butterfly, DIR = +1: exp(-2 pi i pc/r), DIR = -1: exp(+...)
+template <int DIR>
+__device__ __forceinline__ void bfly2(float2* v)
+{
+    float2 a = v[0], b = v[1];
+    v[0] = cadd(a, b);
+    v[1] = csub(a, b);
+}
+template <int DIR>
+__device__ __forceinline__ void bfly3(float2* v)
+{
+    const float h = 0.86602540378443864676f; // sqrt(3)/2
+    float2 a = v[0], b = v[1], c = v[2];
+    float2 t1 = cadd(b, c);
+    float2 t2 = make_float2(a.x - 0.5f * t1.x, a.y - 0.5f * t1.y);
+    float2 d = csub(b, c);
+    float2 t3 = make_float2(h * d.x, h * d.y);
+    v[0] = cadd(a, t1);
+    // forward: y1 = t2 - i t3, y2 = t2 + i t3 ; inverse swaps them
+    float2 m = make_float2(t2.x + t3.y, t2.y - t3.x); // t2 - i t3
+    float2 q = make_float2(t2.x - t3.y, t2.y + t3.x); // t2 + i t3
+    if (DIR > 0) { v[1] = m; v[2] = q; } else { v[1] = q; v[2] = m; }
+}
+template <int DIR>
+__device__ __forceinline__ void bfly4(float2* v)
+{
+    float2 a = v[0], b = v[1], c = v[2], d = v[3];
+    float2 s0 = cadd(a, c), s1 = csub(a, c), s2 = cadd(b, d), s3 = csub(b, d);
+    v[0] = cadd(s0, s2);
+    v[2] = csub(s0, s2);
+    float2 m = make_float2(s1.x + s3.y, s1.y - s3.x); // s1 - i s3
+    float2 q = make_float2(s1.x - s3.y, s1.y + s3.x); // s1 + i s3
+    if (DIR > 0) { v[1] = m; v[3] = q; } else { v[1] = q; v[3] = m; }
+}
+
+// In-place L-point DFT on every line of the tile in shared memory.
+// Element (line l, slot i) lives at s[l*sl + i*se].
+template <int DIR, bool COL>
+__device__ void tile_fft(float2* s, const PassDesc& p, int nl_eff, int sl, int se)
+{
+    const int L = p.L;
+    const float2* __restrict__ wL = p.wL;
+    int nq = (DIR > 0) ? L : 1; // current sub-length n_q
+    for (int qq = 0; qq < p.n_radix; ++qq) {
+        const int q = (DIR > 0) ? qq : (p.n_radix - 1 - qq);
+        const int r = p.radix[q];
+        if (DIR < 0) nq *= r;       // inverse walks the steps backwards: n_q grows
+        const int m = nq / r;       // butterfly stride (slots)
+        const int tws = L / nq;     // W_{n_q}^x = wL[x * tws]
+        const int per_line = L / r;
+        const int nbf = nl_eff * per_line;
+        for (int bf = threadIdx.x; bf < nbf; bf += blockDim.x) {
+            int l, jj;
+            if (COL) { l = bf % nl_eff; jj = bf / nl_eff; } else { jj = bf % per_line; l = bf / per_line; }
+            const int b = jj / m, j = jj - b * m;
+            float2* e = s + l * sl + (b * nq + j) * se;
+            const int step = m * se;
+            float2 v[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if (c < r) v[c] = e[c * step];
+            if (DIR < 0) { // DIT mirror: conj twiddle first
+#pragma unroll
+                for (int c = 1; c < 4; ++c)
+                    if (c < r) v[c] = cmulc(v[c], __ldg(wL + j * c * tws));
+            }
+            if (r == 4) bfly4<DIR>(v);
+            else if (r == 2) bfly2<DIR>(v);
+            else bfly3<DIR>(v);
+            if (DIR > 0) {
+#pragma unroll
+                for (int c = 1; c < 4; ++c)
+                    if (c < r) v[c] = cmul(v[c], __ldg(wL + j * c * tws));
+            }
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if (c < r) e[c * step] = v[c];
+        }
+        __syncthreads();
+        if (DIR > 0) nq = m;
+    }
+}
+
+template <bool COL>
+__global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
+{
+    extern __shared__ float2 s[];
+    __shared__ double red[8];
+
+    // ---- which tile
+    long long t = blockIdx.x;
+    const long long cg = t % p.n_cgroups;
+    t /= p.n_cgroups;
+    const long long m = t % p.n_m;
+    const long long o = t / p.n_m;
+    const long long c0 = cg * p.nl;
+    const int nl_eff = (int)((p.NC - c0) < (long long)p.nl ? (p.NC - c0) : (long long)p.nl);
+    const long long base = o * p.SO + m * p.SM + c0 * p.SCc;
+    const int L = p.L;
+    const int sl = COL ? 1 : L;
+    const int se = COL ? nl_eff : 1;
+    const long long ls = p.SCc, es = p.es;
+    const int total = nl_eff * L;
+    const long long r0 = p.r_from ? m : c0; // boundary-twiddle r of line 0 (x digit: r = c)
+    const int r_per_line = p.r_from ? 0 : 1;
+
+    // ---- load (+ prologue op, + conj boundary twiddle before an inverse DFT)
+    for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+        int l, i;
+        if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+        const long long off = base + l * ls + i * es;
+        float2 v;
+        if (p.load_op == LD_C64) {
+            v = p.field[off];
+        } else if (p.load_op == LD_HEIGHT) {
+            float tt = p.height[off] * p.phase_coef; // Eq. (1) in turns
+            sincospif(2.0f * tt, &v.y, &v.x);        // Eq. (2), E_in = 1
+        } else if (p.load_op == LD_SEED) {
+            float2 u = p.field[off];
+            float g = 2.0f * p.plane_in[off];
+            v = make_float2(g * u.x, g * u.y);
+        } else {
+            v = make_float2(p.plane_in[off], 0.0f);
+        }
+        if (p.tw_b != nullptr && p.fft1_dir < 0) {
+            long long r = r0 + (long long)l * r_per_line;
+            v = cmulc(v, __ldg(p.tw_b + r * p.pi[i]));
+        }
+        s[l * sl + i * se] = v;
+    }
+    __syncthreads();
+
+    if (p.fft1_dir > 0) tile_fft<1, COL>(s, p, nl_eff, sl, se);
+    else tile_fft<-1, COL>(s, p, nl_eff, sl, se);
+
+    // ---- middle op
+    if (p.mid_op == MID_H || p.mid_op == MID_HCONJ || p.mid_op == MID_GAUSS) {
+        const long long row0 = o * p.row_o + m * p.row_m;
+        for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+            int l, i;
+            if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+            const long long row = row0 + i * p.row_i;
+            const long long col = c0 + l;
+            float2 v = s[l * sl + i * se];
+            if (p.mid_op == MID_GAUSS) {
+                float g = p.gx[col] * p.gy[row] * p.scale;
+                v = make_float2(v.x * g, v.y * g);
+            } else {
+                // F4: a = (1/lambda^2 - fx^2) - fy^2 in fp64, the definition's own expression
+                double a = (p.inv_lam2 - p.fx2[col]) - p.fy2[row];
+                if (a >= 0.0) {
+                    double turns = p.z * sqrt(a);
+                    float f = (float)(turns - rint(turns)); // fractional turn, |f| <= 0.5
+                    float sn, cs;
+                    sincospif(2.0f * f, &sn, &cs);
+                    float2 H = make_float2(cs * p.scale, (p.mid_op == MID_H ? sn : -sn) * p.scale);
+                    v = cmul(v, H);
+                } else {
+                    v = make_float2(0.0f, 0.0f); // evanescent: zeroed
+                }
+            }
+            s[l * sl + i * se] = v;
+        }
+        __syncthreads();
+    } else if (p.mid_op == MID_LOSS) {
+        double acc = 0.0;
+        for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+            int l, i;
+            if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+            const long long off = base + l * ls + i * es;
+            float2 v = s[l * sl + i * se];
+            float I = v.x * v.x + v.y * v.y;      // F6
+            float d = I - p.plane_in[off];         // F7
+            acc += (double)d * (double)d;
+            float g = p.seed_coef * d;             // A1: 2 gI = 4 (I - T)/N
+            s[l * sl + i * se] = make_float2(g * v.x, g * v.y);
+            if (p.write_intensity) p.plane_out[off] = I;
+        }
+        // deterministic block reduction: warp shuffle tree, then warp 0 over the 8 partials
+        for (int d = 16; d > 0; d >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, d);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tsum = 0.0;
+            for (int w = 0; w < (int)(blockDim.x >> 5); ++w) tsum += red[w];
+            p.loss_scratch[blockIdx.x] = tsum;
+        }
+        __syncthreads();
+    }
+
+    int last_dir = p.fft1_dir;
+    if (p.fft2_dir != 0) {
+        if (p.fft2_dir > 0) tile_fft<1, COL>(s, p, nl_eff, sl, se);
+        else tile_fft<-1, COL>(s, p, nl_eff, sl, se);
+        last_dir = p.fft2_dir;
+    }
+
+    // ---- store (+ boundary twiddle after a forward DFT, + epilogue op)
+    for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+        int l, i;
+        if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+        const long long off = base + l * ls + i * es;
+        float2 v = s[l * sl + i * se];
+        if (p.tw_b != nullptr && last_dir > 0) {
+            long long r = r0 + (long long)l * r_per_line;
+            v = cmul(v, __ldg(p.tw_b + r * p.pi[i]));
+        }
+        if (p.store_op == ST_C64) {
+            p.field[off] = v;
+        } else if (p.store_op == ST_GRAD || p.store_op == ST_GRAD_ACC) {
+            float tt = p.height[off] * p.phase_coef;
+            float sn, cs;
+            sincospif(2.0f * tt, &sn, &cs); // u0 recomputed, not stored
+            float g = p.grad_coef * (cs * v.y - sn * v.x); // A5: c Im(conj(u0) g)
+            if (p.store_op == ST_GRAD_ACC) g += p.plane_out[off];
+            p.plane_out[off] = g;
+        } else if (p.store_op == ST_C64_INTENSITY) {
+            p.field[off] = v;
+            p.plane_out[off] = v.x * v.x + v.y * v.y;
+        } else {
+            p.plane_out[off] = v.x;
+        }
+    }
+}
+
+cudaError_t launch_tile_pass_generic(const PassDesc& p, cudaStream_t stream)
+{
+    const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
+    if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
+    cudaError_t e;
+    if (p.col_type) {
+        e = cudaFuncSetAttribute(tile_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, p.smem_bytes);
+        if (e != cudaSuccess) return e;
+        tile_pass_kernel<true><<<(unsigned)ntiles, p.threads, p.smem_bytes, stream>>>(p);
+    } else {
+        e = cudaFuncSetAttribute(tile_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, p.smem_bytes);
+        if (e != cudaSuccess) return e;
+        tile_pass_kernel<false><<<(unsigned)ntiles, p.threads, p.smem_bytes, stream>>>(p);
+    }
+    return cudaGetLastError();
+}
+
+// Fixed-order final reduction of the per-CTA loss partials: L = inv_n * sum scratch[0..n)
+__global__ void __launch_bounds__(1024) loss_reduce_kernel(const double* __restrict__ scratch, long long n,
+                                                           double inv_n, double* __restrict__ out)
+{
+    __shared__ double sh[1024];
+    double acc = 0.0;
+    for (long long i = threadIdx.x; i < n; i += 1024) acc += scratch[i];
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int d = 512; d > 0; d >>= 1) {
+        if ((int)threadIdx.x < d) sh[threadIdx.x] += sh[threadIdx.x + d];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0] * inv_n;
+}
+
+cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
+                               cudaStream_t stream)
+{
+    loss_reduce_kernel<<<1, 1024, 0, stream>>>(scratch, n, inv_n, d_loss);
+    return cudaGetLastError();
+}
+
+} // namespace dop

@@ -1,0 +1,316 @@
+// plan.cu -- host-only plan construction: digit factorisation, twiddle and frequency tables
+// (computed in fp64 / long double, rounded once to fp32), pass schedule.  Touches no GPU.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <sstream>
+
+#include "dop_internal.h"
+
+namespace dop {
+
+static const long double kPiL = 3.141592653589793238462643383279502884L;
+
+static bool is_23_smooth(long long n)
+{
+    if (n < 2) return false;
+    while (n % 2 == 0) n /= 2;
+    while (n % 3 == 0) n /= 3;
+    return n == 1;
+}
+
+// radix steps for one digit: 3s first, then 4s, then one 2 if needed
+static std::vector<int> radix_steps(long long L)
+{
+    std::vector<int> r;
+    while (L % 3 == 0) { r.push_back(3); L /= 3; }
+    while (L % 4 == 0) { r.push_back(4); L /= 4; }
+    if (L % 2 == 0) { r.push_back(2); L /= 2; }
+    return r;
+}
+
+// In-place DIF over radices (r_0..r_{t-1}): slot i = sum c_q m_q (m_q = L/(r_0..r_q)) holds
+// output index k = sum c_q (r_0..r_{q-1}).
+static std::vector<int> dif_permutation(long long L, const std::vector<int>& radix)
+{
+    std::vector<int> pi((size_t)L);
+    for (long long i = 0; i < L; ++i) {
+        long long rem = i, m = L, k = 0, w = 1;
+        for (int r : radix) {
+            m /= r;
+            long long c = rem / m;
+            rem -= c * m;
+            k += c * w;
+            w *= r;
+        }
+        pi[(size_t)i] = (int)k;
+    }
+    return pi;
+}
+
+static std::vector<float2> twiddle_table(long long n)
+{
+    std::vector<float2> w((size_t)n);
+    for (long long k = 0; k < n; ++k) {
+        long double a = 2.0L * kPiL * (long double)k / (long double)n;
+        w[(size_t)k] = make_float2((float)cosl(a), (float)(-sinl(a)));
+    }
+    return w;
+}
+
+// Split N into the fewest digits with every digit <= lmax_first (all but the last) and the last
+// <= lmax_last, as balanced as possible.  env_name (if set, e.g. "256,256") overrides.
+static bool split_digits(long long N, long long lmax_first, long long lmax_last, const char* env_name,
+                         std::vector<long long>* out)
+{
+    out->clear();
+    if (const char* e = env_name ? std::getenv(env_name) : nullptr) {
+        std::vector<long long> v;
+        long long prod = 1;
+        std::stringstream ss(e);
+        std::string tok;
+        while (std::getline(ss, tok, ',')) {
+            long long x = std::atoll(tok.c_str());
+            if (x < 2) { v.clear(); break; }
+            v.push_back(x);
+            prod *= x;
+        }
+        if (!v.empty() && prod == N) { *out = v; return true; }
+    }
+    if (N <= lmax_last) { out->push_back(N); return true; }
+    // divisors of N
+    std::vector<long long> divs;
+    for (long long a = 1; a <= N; a *= 2)
+        for (long long b = a; b <= N; b *= 3)
+            if (N % b == 0) divs.push_back(b);
+    std::sort(divs.begin(), divs.end());
+    // two digits
+    long long best = -1, best_cost = 0;
+    for (long long d0 : divs) {
+        long long d1 = N / d0;
+        if (d0 < 2 || d1 < 2 || d0 > lmax_first || d1 > lmax_last) continue;
+        long long cost = std::max(d0, d1);
+        if (best < 0 || cost < best_cost || (cost == best_cost && d0 > best)) { best = d0; best_cost = cost; }
+    }
+    if (best > 0) { out->push_back(best); out->push_back(N / best); return true; }
+    // three digits
+    long long b0 = -1, b1 = -1;
+    best_cost = 0;
+    for (long long d0 : divs)
+        for (long long d1 : divs) {
+            if (d0 < 2 || d1 < 2 || (N / d0) % d1 != 0) continue;
+            long long d2 = N / d0 / d1;
+            if (d2 < 2 || d0 > lmax_first || d1 > lmax_first || d2 > lmax_last) continue;
+            long long cost = std::max(d0, std::max(d1, d2));
+            if (b0 < 0 || cost < best_cost) { b0 = d0; b1 = d1; best_cost = cost; }
+        }
+    if (b0 > 0) { out->push_back(b0); out->push_back(b1); out->push_back(N / b0 / b1); return true; }
+    return false;
+}
+
+static int wl_table_index(dop_plan* p, long long L)
+{
+    for (size_t i = 0; i < p->wl_len.size(); ++i)
+        if (p->wl_len[i] == L) return (int)i;
+    p->wl_len.push_back(L);
+    p->wl_tables.push_back(twiddle_table(L));
+    return (int)p->wl_len.size() - 1;
+}
+
+static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long long>& Ls)
+{
+    Axis& ax = p->ax[a];
+    ax.N = N;
+    ax.dig.resize(Ls.size());
+    long long st = N;
+    for (size_t j = 0; j < Ls.size(); ++j) {
+        Digit& d = ax.dig[j];
+        d.L = Ls[j];
+        st /= Ls[j];
+        d.st = st;
+        d.radix = radix_steps(d.L);
+        if ((int)d.radix.size() > kMaxRadixSteps) return false;
+        d.pi = dif_permutation(d.L, d.radix);
+        d.wl_index = wl_table_index(p, d.L);
+        d.has_twb = (j + 1 < Ls.size());
+        if (d.has_twb) d.twb = twiddle_table(d.L * d.st);
+    }
+    // slot -> true frequency index:  k = sum_j pi_j(p_j) (L_0 .. L_{j-1})
+    ax.kslot.resize((size_t)N);
+    ax.f2.resize((size_t)N);
+    ax.g.resize((size_t)N);
+    const double pitch = p->desc.pitch, sigma = p->desc.prefilter_sigma_px;
+    for (long long s = 0; s < N; ++s) {
+        long long k = 0, w = 1;
+        for (const Digit& d : ax.dig) {
+            long long pj = (s / d.st) % d.L;
+            k += (long long)d.pi[(size_t)pj] * w;
+            w *= d.L;
+        }
+        ax.kslot[(size_t)s] = k;
+        // signed bin, then the definition's own fp64 expressions (F4 / O4)
+        double kb = (double)(k < (N + 1) / 2 ? k : k - N);
+        double f = kb / ((double)N * pitch);
+        ax.f2[(size_t)s] = f * f;
+        double v = kb / (double)N;
+        ax.g[(size_t)s] = (float)std::exp(-2.0 * M_PI * M_PI * sigma * sigma * (v * v));
+    }
+    return true;
+}
+
+static PassTmpl mk(int axis, int digit, int d1, int d2, int ld, int mid, int st, const char* nm, double bpp)
+{
+    PassTmpl t;
+    t.axis = axis; t.digit = digit; t.fft1_dir = d1; t.fft2_dir = d2;
+    t.load_op = ld; t.mid_op = mid; t.store_op = st; t.name = nm; t.bytes_per_point = bpp;
+    return t;
+}
+
+// passes of  F^-1{ mid (x) F{.} }  minus the first forward x digit and the last inverse x digit
+static void sandwich_core(const dop_plan* p, int mid, std::vector<PassTmpl>* out)
+{
+    const int a = (int)p->ax[0].dig.size(), b = (int)p->ax[1].dig.size();
+    for (int j = 1; j < a; ++j) out->push_back(mk(0, j, +1, 0, LD_C64, MID_NONE, ST_C64, "x-fwd", 16));
+    for (int j = 0; j + 1 < b; ++j) out->push_back(mk(1, j, +1, 0, LD_C64, MID_NONE, ST_C64, "y-fwd", 16));
+    out->push_back(mk(1, b - 1, +1, -1, LD_C64, mid, ST_C64,
+                      mid == MID_H ? "y-fwd*H*y-inv" : mid == MID_HCONJ ? "y-fwd*conjH*y-inv" : "y-fwd*G*y-inv", 16));
+    for (int j = b - 2; j >= 0; --j) out->push_back(mk(1, j, -1, 0, LD_C64, MID_NONE, ST_C64, "y-inv", 16));
+    for (int j = a - 1; j >= 1; --j) out->push_back(mk(0, j, -1, 0, LD_C64, MID_NONE, ST_C64, "x-inv", 16));
+}
+
+static void build_schedule(dop_plan* p)
+{
+    const bool l2 = p->desc.loss == DOP_LOSS_L2;
+    const bool wi = l2 && (p->desc.flags & DOP_WRITE_INTENSITY);
+    p->fwd.clear(); p->adj.clear(); p->pre.clear();
+    // forward
+    p->fwd.push_back(mk(0, 0, +1, 0, LD_HEIGHT, MID_NONE, ST_C64, "h->u0,x-fwd", 12));
+    sandwich_core(p, MID_H, &p->fwd);
+    if (l2) {
+        p->fwd.push_back(mk(0, 0, -1, +1, LD_C64, MID_LOSS, ST_C64, "x-inv,|u|^2,loss,seed,x-fwd", wi ? 24 : 20));
+    } else {
+        p->fwd.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_C64_INTENSITY, "x-inv,|u|^2", 20));
+        p->adj.push_back(mk(0, 0, +1, 0, LD_SEED, MID_NONE, ST_C64, "seed,x-fwd", 20));
+    }
+    // adjoint
+    sandwich_core(p, MID_HCONJ, &p->adj);
+    p->adj.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_GRAD, "x-inv,grad", 16));
+    // Gaussian pre-filter (real plane -> real plane through the complex field buffer)
+    if (p->desc.prefilter_sigma_px > 0.0) {
+        p->pre.push_back(mk(0, 0, +1, 0, LD_REAL, MID_NONE, ST_C64, "real,x-fwd", 12));
+        sandwich_core(p, MID_GAUSS, &p->pre);
+        p->pre.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_REAL, "x-inv,real", 12));
+    }
+}
+
+void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
+{
+    const long long nx = p->desc.nx, ny = p->desc.ny;
+    const Digit& g = p->ax[axis].dig[(size_t)digit];
+    const long long L = g.L, st = g.st;
+    d->L = (int)L;
+    d->n_radix = (int)g.radix.size();
+    for (int i = 0; i < d->n_radix; ++i) d->radix[i] = g.radix[(size_t)i];
+    long long nl_target = std::max<long long>(1, p->tile_pts / L);
+    d->row_o = d->row_m = d->row_i = 0;
+    if (axis == 0 && st == 1) { // last x digit: row-type, lines are contiguous runs of L
+        d->col_type = 0;
+        d->es = 1;
+        d->NC = ny * nx / L;
+        d->SCc = L;
+        d->n_m = 1; d->SM = 0; d->n_o = 1; d->SO = 0;
+        d->r_from = 0;
+        d->nl = (int)std::min<long long>(nl_target, d->NC);
+    } else if (axis == 0) { // higher x digit: lines r..r+nl-1 adjacent, elements st apart
+        d->col_type = 1;
+        d->es = st;
+        d->NC = st; d->SCc = 1;
+        d->n_m = nx / (L * st); d->SM = L * st;
+        d->n_o = ny; d->SO = nx;
+        d->r_from = 0;
+        d->nl = (int)std::min<long long>(std::max<long long>(nl_target, 16), st);
+    } else { // y digit: lines are adjacent columns, elements st rows apart
+        d->col_type = 1;
+        d->es = st * nx;
+        d->NC = nx; d->SCc = 1;
+        d->n_m = st; d->SM = nx;
+        d->n_o = ny / (L * st); d->SO = L * st * nx;
+        d->r_from = 1;
+        d->row_o = L * st; d->row_m = 1; d->row_i = st;
+        d->nl = (int)std::min<long long>(std::max<long long>(nl_target, 16), nx);
+    }
+    d->n_cgroups = (d->NC + d->nl - 1) / d->nl;
+    d->smem_bytes = (int)((long long)d->nl * L * (long long)sizeof(float2));
+    d->threads = 256;
+}
+
+dop_status build_plan(dop_plan* p)
+{
+    const dop_plan_desc& d = p->desc;
+    if (!is_23_smooth(d.nx) || !is_23_smooth(d.ny)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (const char* e = std::getenv("DOP_TILE_PTS")) {
+        int v = std::atoi(e);
+        if (v >= 256 && v <= 16384) p->tile_pts = v;
+    }
+    // generic kernel limits: a row-type line <= 8192 points (64 KiB), a column-type digit
+    // <= 512 points (x 16 adjacent lines = 64 KiB)
+    std::vector<long long> lx, ly;
+    if (!split_digits(d.nx, 512, 8192, "DOP_XDIGITS", &lx)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (!split_digits(d.ny, 512, 512, "DOP_YDIGITS", &ly)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (!build_axis(p, 0, d.nx, lx) || !build_axis(p, 1, d.ny, ly)) return DOP_ERR_UNSUPPORTED_SIZE;
+    build_schedule(p);
+    // the MID_LOSS pass is x digit 0
+    PassDesc g{};
+    tile_geometry(p, 0, 0, &g);
+    p->loss_tiles = g.n_cgroups * g.n_m * g.n_o;
+    // workspace: [n_lambda fields][h_eff plane][loss partials]
+    const size_t npts = (size_t)d.nx * (size_t)d.ny;
+    auto align256 = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    p->ws_fields = align256(npts * sizeof(float2)) * (size_t)d.n_lambda;
+    p->ws_heff_off = p->ws_fields;
+    size_t off = p->ws_fields;
+    if (d.prefilter_sigma_px > 0.0) off += align256(npts * sizeof(float));
+    p->ws_loss_off = off;
+    if (d.loss == DOP_LOSS_L2) off += align256((size_t)p->loss_tiles * (size_t)d.n_lambda * sizeof(double));
+    p->ws_bytes = off;
+    return DOP_OK;
+}
+
+std::string describe_plan(const dop_plan* p)
+{
+    std::ostringstream os;
+    const dop_plan_desc& d = p->desc;
+    os << "grid ny=" << d.ny << " nx=" << d.nx << " n_lambda=" << d.n_lambda
+       << " loss=" << (d.loss == DOP_LOSS_L2 ? "L2" : "none") << " prefilter_sigma_px=" << d.prefilter_sigma_px
+       << " workspace_bytes=" << p->ws_bytes << "\n";
+    for (int a = 0; a < 2; ++a) {
+        os << (a == 0 ? "x" : "y") << "-digits:";
+        for (const Digit& g : p->ax[a].dig) {
+            os << " " << g.L << "(st=" << g.st << ",radix=";
+            for (size_t i = 0; i < g.radix.size(); ++i) os << (i ? "." : "") << g.radix[i];
+            os << ")";
+        }
+        os << "\n";
+    }
+    double total = 0;
+    auto dump = [&](const char* tag, const std::vector<PassTmpl>& v) {
+        for (const PassTmpl& t : v) {
+            PassDesc g{};
+            tile_geometry(p, t.axis, t.digit, &g);
+            os << tag << " " << (t.axis == 0 ? "x" : "y") << t.digit << " L=" << g.L << " tile=" << g.nl << "x" << g.L
+               << (g.col_type ? " col" : " row") << " ctas=" << g.n_cgroups * g.n_m * g.n_o
+               << " smem=" << g.smem_bytes << " B/pt=" << t.bytes_per_point << " [" << t.name << "]\n";
+            total += t.bytes_per_point;
+        }
+    };
+    dump("pre", p->pre);
+    dump("fwd", p->fwd);
+    dump("adj", p->adj);
+    dump("pre-adj", p->pre);
+    os << "algorithmic_bytes_per_point=" << total << "\n";
+    return os.str();
+}
+
+} // namespace dop

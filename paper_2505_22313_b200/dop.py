@@ -1,0 +1,183 @@
+"""Thin ctypes binding of the C-ABI library (include/dop.h): same names, argument marshalling
+only -- every step of the hot path runs in the CUDA kernels of libdop.so.  PyTorch appears here
+only as the owner of device memory and streams.  There is no CPU fallback: if libdop.so is
+missing or no sm_100 device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import torch
+
+from . import build as _build
+
+DOP_OK = 0
+DOP_ERR_INVALID_ARG = 1
+DOP_ERR_UNSUPPORTED_SIZE = 2
+DOP_ERR_WORKSPACE = 3
+DOP_ERR_STATE = 4
+DOP_ERR_ARCH = 5
+DOP_ERR_CUDA = 6
+DOP_LOSS_NONE = 0
+DOP_LOSS_L2 = 1
+DOP_WRITE_INTENSITY = 0x1
+
+
+class dop_plan_desc(C.Structure):
+    _fields_ = [
+        ("ny", C.c_int64), ("nx", C.c_int64), ("pitch", C.c_double), ("n_lambda", C.c_int32),
+        ("lambda_", C.POINTER(C.c_double)), ("n_refr", C.POINTER(C.c_double)), ("z", C.c_double),
+        ("loss", C.c_int), ("prefilter_sigma_px", C.c_double), ("flags", C.c_uint32),
+    ]
+
+
+class DopError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {dop_status_string(status)}")
+
+
+def _load() -> C.CDLL:
+    path = _build.LIB
+    if not os.path.exists(path):
+        path = _build.build()
+    lib = C.CDLL(path)
+    vp = C.c_void_p
+    lib.dop_plan_create.argtypes = [C.POINTER(vp), C.POINTER(dop_plan_desc), C.POINTER(C.c_size_t)]
+    lib.dop_plan_create.restype = C.c_int
+    lib.dop_propagate_fwd.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.dop_propagate_fwd.restype = C.c_int
+    lib.dop_propagate_adj.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.dop_propagate_adj.restype = C.c_int
+    lib.dop_plan_destroy.argtypes = [vp]
+    lib.dop_plan_destroy.restype = C.c_int
+    lib.dop_status_string.argtypes = [C.c_int]
+    lib.dop_status_string.restype = C.c_char_p
+    lib.dop_plan_describe.argtypes = [vp, C.c_char_p, C.c_size_t]
+    lib.dop_plan_describe.restype = C.c_size_t
+    lib.dop_plan_launch_count.argtypes = [vp]
+    lib.dop_plan_launch_count.restype = C.c_int64
+    return lib
+
+
+_lib = _load()
+EXPORTS = ("dop_plan_create", "dop_propagate_fwd", "dop_propagate_adj", "dop_plan_destroy",
+           "dop_status_string", "dop_plan_describe", "dop_plan_launch_count")
+
+
+def dop_status_string(status: int) -> str:
+    return _lib.dop_status_string(int(status)).decode()
+
+
+def _ptr(t: Optional[torch.Tensor], dtype, what: str) -> Optional[int]:
+    """device pointer of a contiguous CUDA tensor (None stays NULL)"""
+    if t is None:
+        return None
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise TypeError(f"{what}: need a contiguous CUDA tensor of {dtype}")
+    return t.data_ptr()
+
+
+def dop_plan_create(ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
+                    z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0):
+    """-> (plan handle, workspace_bytes).  Host-only; raises DopError on a bad description."""
+    nl = len(lambdas)
+    lam = (C.c_double * max(nl, 1))(*[float(v) for v in lambdas])
+    nr = (C.c_double * max(nl, 1))(*[float(v) for v in n_refr])
+    d = dop_plan_desc(int(ny), int(nx), float(pitch), nl, lam, nr, float(z), int(loss),
+                      float(prefilter_sigma_px), int(flags))
+    out, ws = C.c_void_p(), C.c_size_t(0)
+    st = _lib.dop_plan_create(C.byref(out), C.byref(d), C.byref(ws))
+    if st != DOP_OK:
+        raise DopError(st, "dop_plan_create")
+    return out, int(ws.value)
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def dop_propagate_fwd(plan, d_height, d_target=None, d_intensity=None, d_loss=None, d_workspace=None,
+                      stream=None) -> None:
+    st = _lib.dop_propagate_fwd(plan, _ptr(d_height, torch.float32, "d_height"),
+                                _ptr(d_target, torch.float32, "d_target"),
+                                _ptr(d_intensity, torch.float32, "d_intensity"),
+                                _ptr(d_loss, torch.float64, "d_loss"),
+                                None if d_workspace is None else d_workspace.data_ptr(), _stream(stream))
+    if st != DOP_OK:
+        raise DopError(st, "dop_propagate_fwd")
+
+
+def dop_propagate_adj(plan, d_height, d_dLdI=None, d_grad_height=None, d_workspace=None, stream=None) -> None:
+    st = _lib.dop_propagate_adj(plan, _ptr(d_height, torch.float32, "d_height"),
+                                _ptr(d_dLdI, torch.float32, "d_dLdI"),
+                                _ptr(d_grad_height, torch.float32, "d_grad_height"),
+                                None if d_workspace is None else d_workspace.data_ptr(), _stream(stream))
+    if st != DOP_OK:
+        raise DopError(st, "dop_propagate_adj")
+
+
+def dop_plan_destroy(plan) -> None:
+    st = _lib.dop_plan_destroy(plan)
+    if st != DOP_OK:
+        raise DopError(st, "dop_plan_destroy")
+
+
+def dop_plan_describe(plan) -> str:
+    n = _lib.dop_plan_describe(plan, None, 0)
+    buf = C.create_string_buffer(n + 1)
+    _lib.dop_plan_describe(plan, buf, n + 1)
+    return buf.value.decode()
+
+
+def dop_plan_launch_count(plan) -> int:
+    return int(_lib.dop_plan_launch_count(plan))
+
+
+class Plan:
+    """Convenience owner of a plan handle and its torch-allocated workspace (marshalling only)."""
+
+    def __init__(self, ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
+                 z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0,
+                 device: str = "cuda:0"):
+        self.ny, self.nx, self.n_lambda, self.loss, self.flags = int(ny), int(nx), len(lambdas), loss, flags
+        self.handle, self.workspace_bytes = dop_plan_create(ny, nx, pitch, lambdas, n_refr, z, loss,
+                                                            prefilter_sigma_px, flags)
+        self.device = torch.device(device)
+        self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
+        self.launches = dop_plan_launch_count(self.handle)
+
+    def describe(self) -> str:
+        return dop_plan_describe(self.handle)
+
+    def fwd(self, height, target=None, intensity=None, loss=None, stream=None) -> None:
+        dop_propagate_fwd(self.handle, height, target, intensity, loss, self.workspace, stream)
+
+    def adj(self, height, dLdI=None, grad=None, stream=None) -> None:
+        dop_propagate_adj(self.handle, height, dLdI, grad, self.workspace, stream)
+
+    def field(self) -> torch.Tensor:
+        """complex64 view [n_lambda, ny, nx] of the workspace fields (valid after a DOP_LOSS_NONE fwd)."""
+        n = self.ny * self.nx
+        stride = (n * 8 + 255) // 256 * 256
+        out = []
+        for l in range(self.n_lambda):
+            raw = self.workspace[l * stride: l * stride + n * 8].view(torch.float32).view(self.ny, self.nx, 2)
+            out.append(torch.view_as_complex(raw))
+        return torch.stack(out)
+
+    def close(self) -> None:
+        if self.handle is not None:
+            dop_plan_destroy(self.handle)
+            self.handle = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
