@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- forward+adjoint ASM throughput on B200 (BASELINE.json metric), with the kernel
+roofline and the fp64 CPU oracle timed beside it.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C1..C5] [--impl reference]
+
+A step = one pass of the whole hot path (dop_propagate_fwd + dop_propagate_adj, every
+wavelength) over one batch of seeded synthetic input.  Default workload: BASELINE.json
+configs[1] (C2: 8192 x 8192, 3 wavelengths).  N > 1 = N independent replicas, one per GPU
+("replicas only"): no data-path collective, weak scaling.
+
+Prints ONE JSON line (rank 0).  `value` = Gpoints/s with inputs resident in HBM; `e2e` = the same
+metric with host buffers (pinned) and host<->device copies inside the timed region; `roofline` =
+achieved algorithmic HBM GB/s of the dominant kernel from per-launch CUDA events; `cpu_baseline`
+= the oracle (oracle/, as it stands) on this box's host cores on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "ASM forward+adjoint Gpoints/s (complex64)"
+UNIT = "Gpoints/s"
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference): bounded sample of the same workload
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(cfg_name: str):
+    """(cfg, sample ny, nx, description): one wavelength on a crop the oracle finishes in ~10-30 s."""
+    from paper_2505_22313_b200 import synth
+    cfg = synth.CONFIGS[cfg_name]
+    ny, nx = min(cfg.ny, 3072), min(cfg.nx, 4096)
+    if cfg.ny == cfg.nx:
+        ny = nx = min(cfg.ny, 4096 if cfg.sigma_px == 0 else 3072)
+    lam = cfg.lambdas[len(cfg.lambdas) // 2]
+    desc = (f"{cfg.name} recipe, top-left {ny}x{nx} crop of the seeded inputs, 1 of {len(cfg.lambdas)} "
+            f"wavelength(s) ({lam * 1e9:.0f} nm), fwd+adj in fp64")
+    return cfg, ny, nx, lam, desc
+
+
+def time_oracle(cfg_name: str, steps: int = 1):
+    """Times oracle forward()+adjoint() as they stand; returns (Gpoints/s, cores, sample text, s/step)."""
+    import numpy as np
+    import torch
+    from oracle import asm_oracle as O
+    from paper_2505_22313_b200 import synth
+    cfg, ny, nx, lam, desc = oracle_sample(cfg_name)
+    small = cfg.scaled(ny, nx)
+    h = synth.make_height(small, "cpu").numpy()
+    T = synth.make_target(small, "cpu").numpy()
+    n_refr = cfg.n_refr[len(cfg.lambdas) // 2]
+    times = []
+    for _ in range(max(1, steps)):
+        t0 = time.perf_counter()
+        O.forward(h, cfg.pitch, [lam], [n_refr], cfg.z, target=T, sigma_px=cfg.sigma_px, keep_field=False)
+        O.adjoint(h, cfg.pitch, [lam], [n_refr], cfg.z, target=T, sigma_px=cfg.sigma_px)
+        times.append(time.perf_counter() - t0)
+    dt = statistics.median(times)
+    return ny * nx / dt / 1e9, O.num_threads(), desc, dt
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(cfg_name: str, pass_name: str):
+    """dram bytes per launch of the dominant pass from the committed ncu capture, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(cfg_name, {}).get(pass_name)
+    except Exception:
+        return None
+
+
+# ------------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2505_22313_b200 import synth
+    cfg = synth.CONFIGS[args.config]
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(args.config, 1)
+    gps, cores, desc, dt = time_oracle(args.config, max(1, min(args.steps, 3)))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gps, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": max(1, min(args.steps, 3)), "warmup": min(args.warmup, 1), "ms_per_step": dt * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": desc},
+        "cpu_baseline": {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": gps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg) -> str:
+    lam = "/".join(f"{l * 1e9:.0f}" for l in cfg.lambdas)
+    s = (f"{cfg.name}: ASM forward+adjoint {cfg.ny}x{cfg.nx}, pitch {cfg.pitch * 1e6:g} um, lambda {lam} nm, "
+         f"z {cfg.z * 1e3:g} mm, L2 loss")
+    if cfg.sigma_px > 0:
+        s += f", Gaussian pre-filter sigma {cfg.sigma_px:g} px"
+    if cfg.write_intensity:
+        s += ", intensity output"
+    return s
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="dop", choices=["dop", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    from paper_2505_22313_b200 import dop, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = synth.CONFIGS[args.config]
+    warmup = max(args.warmup, 3)
+    steps = max(args.steps, 1)
+    flags = dop.DOP_WRITE_INTENSITY if cfg.write_intensity else 0
+    plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, cfg.sigma_px,
+                    flags, device=str(dev))
+    h = synth.make_height(cfg, dev)
+    T = synth.make_target(cfg, dev)
+    grad = torch.empty_like(h)
+    inten = torch.empty((len(cfg.lambdas), cfg.ny, cfg.nx), dtype=torch.float32, device=dev) if flags else None
+    loss = torch.zeros(1, dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream()
+    points = cfg.points
+
+    def step():
+        plan.fwd(h, T, inten, loss)
+        plan.adj(h, None, grad)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        step()
+    barrier()
+
+    # ---- timed region: K steps, inputs resident in HBM, CUDA events on the launching stream
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / steps
+    value = world * points / (ms_per_step * 1e-3) / 1e9
+    loss_value = float(loss.item())
+
+    # ---- per-launch CUDA events (same stream, same steps): the roofline of the dominant kernel
+    dop.dop_plan_set_profiling(plan.handle, True)
+    acc = {}
+    order = []
+    prof_steps = min(steps, 10)
+    for _ in range(prof_steps):
+        step()
+        torch.cuda.synchronize()
+        for name, t_ms, bpp in dop.dop_plan_get_pass_times(plan.handle):
+            key = name.split(":", 1)[1] if ":" in name else name  # merge fwd/adj launches of the same kernel+digit
+            if key not in acc:
+                acc[key] = [0.0, 0, bpp, 0.0]
+                order.append(key)
+            acc[key][0] += t_ms
+            acc[key][1] += 1
+            acc[key][3] += bpp
+    dop.dop_plan_set_profiling(plan.handle, False)
+    peak, peak_src = measured_peak_gbs()
+    npts_plane = cfg.ny * cfg.nx
+    passes = []
+    for key in order:
+        tot, cnt, _, bsum = acc[key]
+        avg_ms = tot / cnt
+        gbs = (bsum / cnt) * npts_plane / (avg_ms * 1e-3) / 1e9 if avg_ms > 0 else 0.0
+        passes.append({"pass": key, "launches_per_step": cnt / prof_steps, "avg_ms": round(avg_ms, 4),
+                       "bytes_per_point": bsum / cnt, "GBps": round(gbs, 1), "frac": round(gbs / peak, 4),
+                       "share": 0.0})
+    total_prof = sum(acc[k][0] for k in order)
+    for p_, key in zip(passes, order):
+        p_["share"] = round(acc[key][0] / total_prof, 4)
+    dom = max(passes, key=lambda p_: p_["share"])
+    step_bytes = sum(acc[k][3] for k in order) / prof_steps * npts_plane
+    roofline = {
+        "bound": "hbm", "kernel": dom["pass"], "achieved": dom["GBps"], "peak": peak, "unit": "GB/s",
+        "frac": round(dom["GBps"] / peak, 4), "traffic": ncu_traffic(args.config, dom["pass"]),
+        "peak_source": peak_src, "bytes_per_launch": dom["bytes_per_point"] * npts_plane,
+        "avg_launch_ms": dom["avg_ms"], "share_of_step": dom["share"],
+        "whole_step": {"algorithmic_bytes_per_point": step_bytes / points,
+                       "GBps": round(step_bytes / (ms_per_step * 1e-3) / 1e9, 1),
+                       "frac": round(step_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 4),
+                       "fused_minimum_bytes_per_point": 80 + (4 if cfg.write_intensity else 0) + (36 if cfg.sigma_px > 0 else 0),
+                       },
+        "passes": passes,
+    }
+
+    # ---- e2e: host (pinned) buffers, H2D of h and T and D2H of grad + loss inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        h_host = h.cpu().pin_memory()
+        T_host = T.cpu().pin_memory()
+        g_host = torch.empty_like(h_host).pin_memory()
+        l_host = torch.zeros(1, dtype=torch.float64).pin_memory()
+        i_host = torch.empty(inten.shape, dtype=torch.float32).pin_memory() if inten is not None else None
+        e2e_steps = max(1, min(steps, 5))
+
+        def e2e_step():
+            h.copy_(h_host, non_blocking=True)
+            T.copy_(T_host, non_blocking=True)
+            step()
+            g_host.copy_(grad, non_blocking=True)
+            l_host.copy_(loss, non_blocking=True)
+            if i_host is not None:
+                i_host.copy_(inten, non_blocking=True)
+
+        e2e_step()
+        barrier()
+        e0.record(stream)
+        for _ in range(e2e_steps):
+            e2e_step()
+        e1.record(stream)
+        barrier()
+        ms2 = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms2], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms2 = float(t.item())
+        h2d = h_host.numel() * 4 + T_host.numel() * 4
+        d2h = g_host.numel() * 4 + 8 + (i_host.numel() * 4 if i_host is not None else 0)
+        e2e = {"value": world * points / (ms2 / e2e_steps * 1e-3) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+               "ms_per_step": ms2 / e2e_steps}
+        del h_host, T_host, g_host, i_host
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        gps, cores, desc, dt = time_oracle(args.config, 1)
+        cpu = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+               "seconds": round(dt, 2)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "c64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "points_per_step": points, "parallelism": f"replicas x{world}",
+                       "l2": "working set (>= 1.5 GiB) larger than the 126 MB L2; no flush between steps"
+                       if points * 8 > 4 * 126e6 else "working set fits L2 (latency-bound config)",
+                       "loss": loss_value},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": plan.launches * steps, "roofline": roofline,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    plan.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

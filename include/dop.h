@@ -139,6 +139,20 @@ size_t dop_plan_describe(const dop_plan* plan, char* buf, size_t len);
 /* Number of kernel launches one dop_propagate_fwd + dop_propagate_adj pair enqueues. */
 int64_t dop_plan_launch_count(const dop_plan* plan);
 
+/*
+ * Per-launch timing (measurement aid for bench.py's roofline line; off by default).
+ * dop_plan_set_profiling(plan, 1): every later dop_propagate_fwd/adj records one CUDA event
+ * pair around each kernel it enqueues, on the caller's stream (events are owned by the plan;
+ * the slots restart at every dop_propagate_fwd).  dop_plan_get_pass_times synchronises those
+ * events and writes, for launch i of the last fwd(+adj): ms[i] = its device time in
+ * milliseconds and bytes_per_point[i] = its algorithmic HBM bytes per grid point (either array
+ * may be NULL); returns the number of recorded launches (<= n are written).
+ * dop_plan_pass_name(plan, i): static-lifetime-of-plan name of recorded launch i, or "".
+ */
+dop_status dop_plan_set_profiling(dop_plan* plan, int enable);
+int64_t dop_plan_get_pass_times(dop_plan* plan, float* ms, double* bytes_per_point, int64_t n);
+const char* dop_plan_pass_name(const dop_plan* plan, int64_t i);
+
 #ifdef __cplusplus
 }
 #endif

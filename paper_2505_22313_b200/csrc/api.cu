@@ -140,12 +140,39 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     return d;
 }
 
-dop_status run(const dop_plan* p, const std::vector<PassTmpl>& sched, int lam, const Buffers& b, char* ws,
-               cudaStream_t st)
+// profiling slot for the next launch: records the start event, returns the slot (or -1)
+long long prof_begin(dop_plan* p, const std::string& name, double bpp, cudaStream_t st)
+{
+    if (!p->profiling) return -1;
+    const size_t i = p->prof_n++;
+    if (i >= p->ev_start.size()) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { p->prof_n--; return -1; }
+        p->ev_start.push_back(a);
+        p->ev_stop.push_back(b);
+        p->prof_name.emplace_back();
+        p->prof_bpp.push_back(0.0);
+    }
+    p->prof_name[i] = name;
+    p->prof_bpp[i] = bpp;
+    cudaEventRecord(p->ev_start[i], st);
+    return (long long)i;
+}
+void prof_end(dop_plan* p, long long slot, cudaStream_t st)
+{
+    if (slot >= 0) cudaEventRecord(p->ev_stop[(size_t)slot], st);
+}
+
+dop_status run(dop_plan* p, const std::vector<PassTmpl>& sched, int lam, const Buffers& b, char* ws,
+               cudaStream_t st, const char* tag)
 {
     for (const PassTmpl& t : sched) {
         PassDesc d = resolve(p, t, lam, b, ws);
-        if (launch_tile_pass(d, st) != cudaSuccess) return DOP_ERR_CUDA;
+        long long slot = prof_begin(p, std::string(tag) + ":" + (t.axis == 0 ? "x" : "y") + std::to_string(t.digit) + ":" + t.name,
+                                    t.bytes_per_point, st);
+        cudaError_t e = launch_tile_pass(d, st);
+        prof_end(p, slot, st);
+        if (e != cudaSuccess) return DOP_ERR_CUDA;
     }
     return DOP_OK;
 }
@@ -200,6 +227,7 @@ dop_status dop_propagate_fwd(dop_plan* p, const float* d_height, const float* d_
     dop_status s = ensure_device(p);
     if (s != DOP_OK) return s;
     p->state = 0;
+    p->prof_n = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
     Buffers b;
@@ -211,16 +239,18 @@ dop_status dop_propagate_fwd(dop_plan* p, const float* d_height, const float* d_
         Buffers pb;
         pb.real_src = d_height;
         pb.real_dst = heff;
-        if ((s = run(p, p->pre, 0, pb, ws, st)) != DOP_OK) return s;
+        if ((s = run(p, p->pre, 0, pb, ws, st, "pre")) != DOP_OK) return s;
         b.height = heff;
     }
     for (int lam = 0; lam < p->desc.n_lambda; ++lam)
-        if ((s = run(p, p->fwd, lam, b, ws, st)) != DOP_OK) return s;
+        if ((s = run(p, p->fwd, lam, b, ws, st, "fwd")) != DOP_OK) return s;
     if (l2 && d_loss != nullptr) {
         const double inv_n = 1.0 / ((double)p->desc.nx * (double)p->desc.ny);
-        if (launch_loss_reduce((const double*)(ws + p->ws_loss_off), p->loss_tiles * p->desc.n_lambda, inv_n, d_loss,
-                               st) != cudaSuccess)
-            return DOP_ERR_CUDA;
+        long long slot = prof_begin(p, "fwd:loss-reduce", 0.0, st);
+        cudaError_t e = launch_loss_reduce((const double*)(ws + p->ws_loss_off), p->loss_tiles * p->desc.n_lambda,
+                                           inv_n, d_loss, st);
+        prof_end(p, slot, st);
+        if (e != cudaSuccess) return DOP_ERR_CUDA;
     }
     p->state = 1;
     return DOP_OK;
@@ -243,12 +273,12 @@ dop_status dop_propagate_adj(dop_plan* p, const float* d_height, const float* d_
     b.dLdI = d_dLdI;
     b.grad = d_grad_height;
     for (int lam = 0; lam < p->desc.n_lambda; ++lam)
-        if ((s = run(p, p->adj, lam, b, ws, st)) != DOP_OK) return s;
+        if ((s = run(p, p->adj, lam, b, ws, st, "adj")) != DOP_OK) return s;
     if (!p->pre.empty()) { // A6: the Gaussian spectrum is real and even, so the filter is self-adjoint
         Buffers pb;
         pb.real_src = d_grad_height;
         pb.real_dst = d_grad_height;
-        if ((s = run(p, p->pre, 0, pb, ws, st)) != DOP_OK) return s;
+        if ((s = run(p, p->pre, 0, pb, ws, st, "pre-adj")) != DOP_OK) return s;
     }
     return DOP_OK;
 }
@@ -257,6 +287,8 @@ dop_status dop_plan_destroy(dop_plan* p)
 {
     if (p == nullptr) return DOP_ERR_INVALID_ARG;
     if (p->d_arena != nullptr) cudaFree(p->d_arena);
+    for (cudaEvent_t e : p->ev_start) cudaEventDestroy(e);
+    for (cudaEvent_t e : p->ev_stop) cudaEventDestroy(e);
     delete p;
     return DOP_OK;
 }
@@ -293,6 +325,36 @@ int64_t dop_plan_launch_count(const dop_plan* p)
     int64_t n = (int64_t)(p->fwd.size() + p->adj.size()) * p->desc.n_lambda + 2 * (int64_t)p->pre.size();
     if (p->desc.loss == DOP_LOSS_L2) n += 1;
     return n;
+}
+
+dop_status dop_plan_set_profiling(dop_plan* p, int enable)
+{
+    if (p == nullptr) return DOP_ERR_INVALID_ARG;
+    p->profiling = enable != 0;
+    p->prof_n = 0;
+    return DOP_OK;
+}
+
+int64_t dop_plan_get_pass_times(dop_plan* p, float* ms, double* bytes_per_point, int64_t n)
+{
+    if (p == nullptr) return 0;
+    for (size_t i = 0; i < p->prof_n && (int64_t)i < n; ++i) {
+        if (ms != nullptr) {
+            float t = 0.0f;
+            if (cudaEventSynchronize(p->ev_stop[i]) != cudaSuccess ||
+                cudaEventElapsedTime(&t, p->ev_start[i], p->ev_stop[i]) != cudaSuccess)
+                t = -1.0f;
+            ms[i] = t;
+        }
+        if (bytes_per_point != nullptr) bytes_per_point[i] = p->prof_bpp[i];
+    }
+    return (int64_t)p->prof_n;
+}
+
+const char* dop_plan_pass_name(const dop_plan* p, int64_t i)
+{
+    if (p == nullptr || i < 0 || (size_t)i >= p->prof_n) return "";
+    return p->prof_name[(size_t)i].c_str();
 }
 
 } // extern "C"

@@ -150,6 +150,12 @@ struct dop_plan {
     float* d_g[2] = {nullptr, nullptr};
     std::vector<size_t> pi_off[2];
     int state = 0; // 1 after a successful fwd
+    // per-launch profiling (dop_plan_set_profiling)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev_start, ev_stop;
+    std::vector<std::string> prof_name;
+    std::vector<double> prof_bpp;
+    size_t prof_n = 0;
 };
 
 namespace dop {

@@ -59,12 +59,19 @@ def _load() -> C.CDLL:
     lib.dop_plan_describe.restype = C.c_size_t
     lib.dop_plan_launch_count.argtypes = [vp]
     lib.dop_plan_launch_count.restype = C.c_int64
+    lib.dop_plan_set_profiling.argtypes = [vp, C.c_int]
+    lib.dop_plan_set_profiling.restype = C.c_int
+    lib.dop_plan_get_pass_times.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_double), C.c_int64]
+    lib.dop_plan_get_pass_times.restype = C.c_int64
+    lib.dop_plan_pass_name.argtypes = [vp, C.c_int64]
+    lib.dop_plan_pass_name.restype = C.c_char_p
     return lib
 
 
 _lib = _load()
 EXPORTS = ("dop_plan_create", "dop_propagate_fwd", "dop_propagate_adj", "dop_plan_destroy",
-           "dop_status_string", "dop_plan_describe", "dop_plan_launch_count")
+           "dop_status_string", "dop_plan_describe", "dop_plan_launch_count",
+           "dop_plan_set_profiling", "dop_plan_get_pass_times", "dop_plan_pass_name")
 
 
 def dop_status_string(status: int) -> str:
@@ -136,6 +143,21 @@ def dop_plan_describe(plan) -> str:
 
 def dop_plan_launch_count(plan) -> int:
     return int(_lib.dop_plan_launch_count(plan))
+
+
+def dop_plan_set_profiling(plan, enable: bool) -> None:
+    st = _lib.dop_plan_set_profiling(plan, int(bool(enable)))
+    if st != DOP_OK:
+        raise DopError(st, "dop_plan_set_profiling")
+
+
+def dop_plan_get_pass_times(plan):
+    """-> list of (name, ms, algorithmic bytes per point) for every launch of the last fwd(+adj)."""
+    n = int(_lib.dop_plan_get_pass_times(plan, None, None, 0))
+    ms = (C.c_float * max(n, 1))()
+    bpp = (C.c_double * max(n, 1))()
+    _lib.dop_plan_get_pass_times(plan, ms, bpp, n)
+    return [(_lib.dop_plan_pass_name(plan, i).decode(), float(ms[i]), float(bpp[i])) for i in range(n)]
 
 
 class Plan:
