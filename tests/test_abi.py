@@ -1,0 +1,129 @@
+"""The C-ABI boundary (include/dop.h) without a GPU: libdop.so loads, exports every symbol the
+header declares, dop_plan_create validates and plans on the host alone, and the propagate calls
+fail loudly (never fall back to a CPU path) when no sm_100 device is present."""
+import ctypes as C
+import os
+import re
+
+import pytest
+import torch
+
+from paper_2505_22313_b200 import build as dop_build
+from paper_2505_22313_b200 import dop
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "dop.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(dop_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    names = _declared_symbols()
+    assert {"dop_plan_create", "dop_propagate_fwd", "dop_propagate_adj", "dop_plan_destroy"} <= set(names)
+    lib = C.CDLL(dop_build.build())
+    for n in names:
+        assert hasattr(lib, n), n
+    assert set(names) == set(dop.EXPORTS)
+
+
+def test_status_strings():
+    for s in range(0, 7):
+        assert dop.dop_status_string(s).startswith("DOP_")
+    assert "UNKNOWN" in dop.dop_status_string(99)
+
+
+@pytest.mark.parametrize("ny,nx", [(1024, 1024), (8192, 8192), (16384, 16384), (65536, 65536), (98304, 65536),
+                                   (2, 2), (3, 2), (2, 3), (6, 4), (384, 512), (1536, 2048), (19683, 4)])
+def test_plan_create_supported_sizes(ny, nx):
+    plan, ws = dop.dop_plan_create(ny, nx, 0.25e-6, [550e-9], [1.5], 1e-3)
+    try:
+        assert ws >= ny * nx * 8
+        text = dop.dop_plan_describe(plan)
+        assert f"ny={ny} nx={nx}" in text
+        # every digit product reproduces the axis length
+        for axis, n in (("x", nx), ("y", ny)):
+            line = [l for l in text.splitlines() if l.startswith(f"{axis}-digits:")][0]
+            prod = 1
+            for m in re.findall(r" (\d+)\(st=", line):
+                prod *= int(m)
+            assert prod == n
+        assert dop.dop_plan_launch_count(plan) >= 5
+    finally:
+        dop.dop_plan_destroy(plan)
+
+
+def test_workspace_sizes_fit_the_memory_plan():
+    """SURVEY.md 8(a) memory plan: C5 = 48 GiB field + 3 x 24 GiB planes < 180 GB; C4 with I output."""
+    plan, ws = dop.dop_plan_create(98304, 65536, 0.25e-6, [550e-9], [1.5], 0.1)
+    dop.dop_plan_destroy(plan)
+    n = 98304 * 65536
+    assert ws < n * 8 + (64 << 20)
+    assert ws + 3 * n * 4 < 180e9
+    plan, ws = dop.dop_plan_create(65536, 65536, 0.25e-6, [550e-9], [1.5], 0.05, flags=dop.DOP_WRITE_INTENSITY)
+    dop.dop_plan_destroy(plan)
+    assert ws + 4 * (1 << 32) * 4 < 180e9
+    # pre-filter adds one fp32 plane, n_lambda multiplies the fields
+    plan, ws3 = dop.dop_plan_create(512, 512, 0.5e-6, [450e-9, 550e-9, 650e-9], [1.5] * 3, 1e-3)
+    dop.dop_plan_destroy(plan)
+    plan, ws1 = dop.dop_plan_create(512, 512, 0.5e-6, [550e-9], [1.5], 1e-3)
+    dop.dop_plan_destroy(plan)
+    plan, wsp = dop.dop_plan_create(512, 512, 0.5e-6, [550e-9], [1.5], 1e-3, prefilter_sigma_px=3.0)
+    dop.dop_plan_destroy(plan)
+    assert ws3 - ws1 >= 2 * 512 * 512 * 8 and wsp - ws1 >= 512 * 512 * 4
+
+
+@pytest.mark.parametrize("kw,status", [
+    (dict(ny=1024, nx=1000), dop.DOP_ERR_UNSUPPORTED_SIZE),     # 1000 = 2^3 5^3
+    (dict(ny=1, nx=64), dop.DOP_ERR_UNSUPPORTED_SIZE),
+    (dict(ny=64, nx=0), dop.DOP_ERR_UNSUPPORTED_SIZE),
+    (dict(ny=7, nx=64), dop.DOP_ERR_UNSUPPORTED_SIZE),
+    (dict(pitch=0.0), dop.DOP_ERR_INVALID_ARG),
+    (dict(pitch=float("nan")), dop.DOP_ERR_INVALID_ARG),
+    (dict(lambdas=[]), dop.DOP_ERR_INVALID_ARG),
+    (dict(lambdas=[-1.0]), dop.DOP_ERR_INVALID_ARG),
+    (dict(z=float("inf")), dop.DOP_ERR_INVALID_ARG),
+    (dict(loss=7), dop.DOP_ERR_INVALID_ARG),
+    (dict(prefilter_sigma_px=-1.0), dop.DOP_ERR_INVALID_ARG),
+    (dict(flags=0x80), dop.DOP_ERR_INVALID_ARG),
+])
+def test_plan_create_rejects_bad_descriptions(kw, status):
+    args = dict(ny=64, nx=64, pitch=1e-6, lambdas=[550e-9], n_refr=[1.5], z=1e-3)
+    args.update(kw)
+    if len(args["n_refr"]) != len(args["lambdas"]):
+        args["n_refr"] = [1.5] * len(args["lambdas"])
+    with pytest.raises(dop.DopError) as e:
+        dop.dop_plan_create(**args)
+    assert e.value.status == status
+
+
+def test_null_arguments():
+    lib = dop._lib
+    assert lib.dop_plan_create(None, None, None) == dop.DOP_ERR_INVALID_ARG
+    assert lib.dop_plan_destroy(None) == dop.DOP_ERR_INVALID_ARG
+    assert lib.dop_propagate_fwd(None, None, None, None, None, None, None) == dop.DOP_ERR_INVALID_ARG
+    assert lib.dop_propagate_adj(None, None, None, None, None, None) == dop.DOP_ERR_INVALID_ARG
+    plan, _ = dop.dop_plan_create(64, 64, 1e-6, [550e-9], [1.5], 1e-3)
+    try:
+        fake = C.c_void_p(4096)
+        # adj before fwd
+        assert lib.dop_propagate_adj(plan, fake, None, fake, fake, None) == dop.DOP_ERR_STATE
+        # L2 needs a target; missing workspace
+        assert lib.dop_propagate_fwd(plan, fake, None, None, None, fake, None) == dop.DOP_ERR_INVALID_ARG
+        assert lib.dop_propagate_fwd(plan, fake, fake, None, None, None, None) == dop.DOP_ERR_WORKSPACE
+    finally:
+        dop.dop_plan_destroy(plan)
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_no_cpu_fallback_without_a_device():
+    """Without a CUDA device the propagate call must fail (DOP_ERR_CUDA / DOP_ERR_ARCH), never compute."""
+    plan, _ = dop.dop_plan_create(64, 64, 1e-6, [550e-9], [1.5], 1e-3)
+    try:
+        fake = C.c_void_p(4096)
+        st = dop._lib.dop_propagate_fwd(plan, fake, fake, None, None, fake, None)
+        assert st in (dop.DOP_ERR_CUDA, dop.DOP_ERR_ARCH)
+    finally:
+        dop.dop_plan_destroy(plan)

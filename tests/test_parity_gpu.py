@@ -1,0 +1,323 @@
+"""Parity of the CUDA path (through the C-ABI, via the thin binding) against the fp64 oracle,
+element by element on the same seeded inputs (the same bytes go to both sides).
+
+Bars (BASELINE.json north_star): rel-L2 <= 1e-5 and max-abs/peak <= 1e-4
+for the complex64 field u and the intensity I; this suite applies the same two bars to dL/dh and
+|L - L_ref|/|L_ref| <= 1e-5 to the loss.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from conftest import max_rel_peak, rel_l2
+from oracle import asm_oracle as orc
+from paper_2505_22313_b200 import dop, synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_L2, TOL_PEAK, TOL_LOSS = 1e-5, 1e-4, 1e-5
+DEV = "cuda:0"
+
+
+def check(a, b, what):
+    e2, ep = rel_l2(a, b), max_rel_peak(a, b)
+    assert e2 <= TOL_L2 and ep <= TOL_PEAK, f"{what}: rel-L2 {e2:.3e}, max-abs/peak {ep:.3e}"
+    return e2, ep
+
+
+def run_l2(cfg, h, T, lambdas=None, n_refr=None, write_i=True):
+    lambdas = cfg.lambdas if lambdas is None else lambdas
+    n_refr = cfg.n_refr if n_refr is None else n_refr
+    flags = dop.DOP_WRITE_INTENSITY if write_i else 0
+    plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, lambdas, n_refr, cfg.z, dop.DOP_LOSS_L2, cfg.sigma_px, flags, DEV)
+    inten = torch.full((len(lambdas), cfg.ny, cfg.nx), float("nan"), dtype=torch.float32, device=DEV) if write_i else None
+    grad = torch.full_like(h, float("nan"))
+    loss = torch.full((1,), float("nan"), dtype=torch.float64, device=DEV)
+    plan.fwd(h, T, inten, loss)
+    plan.adj(h, None, grad)
+    torch.cuda.synchronize()
+    out = (None if inten is None else inten.cpu().numpy(), float(loss.item()), grad.cpu().numpy())
+    plan.close()
+    return out
+
+
+def oracle_l2(cfg, h, T, lambdas=None, n_refr=None):
+    lambdas = cfg.lambdas if lambdas is None else lambdas
+    n_refr = cfg.n_refr if n_refr is None else n_refr
+    hn, Tn = h.cpu().numpy(), T.cpu().numpy()
+    f = orc.forward(hn, cfg.pitch, lambdas, n_refr, cfg.z, target=Tn, sigma_px=cfg.sigma_px, keep_field=False)
+    g = orc.adjoint(hn, cfg.pitch, lambdas, n_refr, cfg.z, target=Tn, sigma_px=cfg.sigma_px)
+    return f["I"], f["loss"], g
+
+
+# ------------------------------------------------------------------------------------------------
+# small and medium grids: several tiles, ragged tails, radix 3, one- two- and three-digit axes
+# ------------------------------------------------------------------------------------------------
+SHAPES = [(2, 2), (2, 3), (3, 2), (4, 6), (16, 16), (48, 36), (27, 64), (96, 128), (384, 512), (1024, 768),
+          (1536, 2048), (2048, 1024), (243, 256), (4096, 512), (512, 16384), (18, 20736)]
+
+
+@pytest.mark.parametrize("ny,nx", SHAPES)
+def test_field_intensity_and_caller_seeded_adjoint(ny, nx):
+    """DOP_LOSS_NONE: field u (read from the workspace), I, then adj with a caller-supplied dL/dI."""
+    cfg = synth.CONFIGS["C4"].scaled(ny, nx)          # pitch 0.25 um: evanescent bins present
+    z = 2e-3
+    lambdas, n_refr = (550e-9, 633e-9), (1.5, 1.47)
+    h = synth.make_height(cfg, DEV)
+    dLdI = synth.uniform_plane(77, 5, 2 * ny, nx, DEV).view(2, ny, nx).contiguous() - 0.5
+    plan = dop.Plan(ny, nx, cfg.pitch, lambdas, n_refr, z, dop.DOP_LOSS_NONE, 0.0, 0, DEV)
+    inten = torch.empty((2, ny, nx), dtype=torch.float32, device=DEV)
+    grad = torch.empty_like(h)
+    plan.fwd(h, None, inten, None)
+    torch.cuda.synchronize()
+    u = plan.field().cpu().numpy()
+    plan.adj(h, dLdI, grad)
+    torch.cuda.synchronize()
+    plan.close()
+    hn = h.cpu().numpy()
+    ref = orc.forward(hn, cfg.pitch, lambdas, n_refr, z)
+    check(u, ref["u"], "field u")
+    check(inten.cpu().numpy(), ref["I"], "intensity")
+    gref = orc.adjoint(hn, cfg.pitch, lambdas, n_refr, z, dLdI=dLdI.cpu().numpy())
+    check(grad.cpu().numpy(), gref, "dL/dh")
+
+
+@pytest.mark.parametrize("ny,nx", [(2, 2), (6, 4), (96, 128), (384, 512), (1536, 1024), (512, 6144)])
+def test_fused_l2_loss_path(ny, nx):
+    # C2's blurred-noise recipe degenerates (zero range) on grids smaller than its blur: tiny grids use C1's
+    cfg = synth.CONFIGS["C2" if ny * nx >= 4096 else "C1"].scaled(ny, nx)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I, L, g = run_l2(cfg, h, T)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+    # without the optional intensity output the loss and gradient are unchanged
+    _, L2, g2 = run_l2(cfg, h, T, write_i=False)
+    assert L2 == L and np.array_equal(g2, g)
+
+
+@pytest.mark.parametrize("ny,nx", [(48, 64), (384, 512), (1024, 1536)])
+def test_prefilter_path(ny, nx):
+    cfg = synth.CONFIGS["C3"].scaled(ny, nx)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    assert len(np.unique(h.cpu().numpy())) <= 256     # 256 gray levels
+    I, L, g = run_l2(cfg, h, T)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
+@pytest.mark.parametrize("env", [{"DOP_XDIGITS": "16,8", "DOP_YDIGITS": "4,12"},
+                                 {"DOP_XDIGITS": "2,4,16", "DOP_YDIGITS": "3,4,4"},
+                                 {"DOP_XDIGITS": "128", "DOP_YDIGITS": "48"}])
+def test_every_digit_decomposition_gives_the_same_answer(env, monkeypatch):
+    """The multi-pass (four-step) decomposition used for 65536-point lines, forced on a small grid."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    cfg = synth.CONFIGS["C5"].scaled(48, 128)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I, L, g = run_l2(cfg, h, T)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
+def test_degenerate_inputs():
+    """z = 0 (identity on a grid without evanescent bins), flat height (plane wave), negative z."""
+    cfg = synth.CONFIGS["C1"].scaled(64, 96)
+    h = synth.make_height(cfg, DEV)
+    plan = dop.Plan(64, 96, cfg.pitch, cfg.lambdas, cfg.n_refr, 0.0, dop.DOP_LOSS_NONE, 0.0, 0, DEV)
+    inten = torch.empty((1, 64, 96), dtype=torch.float32, device=DEV)
+    plan.fwd(h, None, inten, None)
+    torch.cuda.synchronize()
+    u = plan.field().cpu().numpy()[0]
+    plan.close()
+    u0 = orc.phase_field(h.cpu().numpy(), cfg.lambdas[0], cfg.n_refr[0])
+    check(u, u0, "z=0 identity")
+    assert np.abs(inten.cpu().numpy() - 1).max() < 1e-5
+    flat = torch.full((64, 96), 0.3e-6, dtype=torch.float32, device=DEV)
+    for z in (1e-3, -1e-3):
+        plan = dop.Plan(64, 96, cfg.pitch, cfg.lambdas, cfg.n_refr, z, dop.DOP_LOSS_NONE, 0.0, 0, DEV)
+        plan.fwd(flat, None, inten, None)
+        torch.cuda.synchronize()
+        u = plan.field().cpu().numpy()[0]
+        plan.close()
+        lam, n = cfg.lambdas[0], cfg.n_refr[0]
+        expect = np.exp(2j * np.pi * (n - 1) * float(flat[0, 0].item()) / lam) * np.exp(2j * np.pi * z / lam)
+        assert np.abs(u - expect).max() < 1e-5          # plane wave picks up e^{ikz} (P-b)
+
+
+def test_state_and_argument_errors_on_device():
+    cfg = synth.CONFIGS["C1"].scaled(32, 32)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    plan = dop.Plan(32, 32, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, 0.0, 0, DEV)
+    grad = torch.empty_like(h)
+    with pytest.raises(dop.DopError) as e:
+        plan.adj(h, None, grad)
+    assert e.value.status == dop.DOP_ERR_STATE
+    with pytest.raises(dop.DopError) as e:
+        plan.fwd(h, None, None, None)                   # L2 needs a target
+    assert e.value.status == dop.DOP_ERR_INVALID_ARG
+    plan.fwd(h, T, None, None)                          # d_loss may be NULL
+    plan.adj(h, None, grad)
+    with pytest.raises(dop.DopError):
+        plan.adj(h, None, grad)                         # one adj per fwd
+    torch.cuda.synchronize()
+    plan.close()
+
+
+def test_repeatable_bitwise():
+    cfg = synth.CONFIGS["C2"].scaled(768, 1024)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    a = run_l2(cfg, h, T)
+    b = run_l2(cfg, h, T)
+    assert np.array_equal(a[0], b[0]) and a[1] == b[1] and np.array_equal(a[2], b[2])
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json configurations at full size, in the launch configuration bench.py times
+# ------------------------------------------------------------------------------------------------
+def test_C1_full_size_against_the_oracle():
+    cfg = synth.CONFIGS["C1"]
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I, L, g = run_l2(cfg, h, T)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "C1 intensity")
+    check(g, gr, "C1 dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
+def tiled_case(name, py, px, lambdas_idx=None):
+    """Pin P-k: tile a py x px problem R times; spectrum lives on multiples of R where
+    the big grid's H equals the small grid's, so I_big = tile(I_small), L_big = L_small,
+    Ry Rx grad_big = tile(grad_small).  The small problem comes from the full oracle."""
+    cfg = synth.CONFIGS[name]
+    ry, rx = cfg.ny // py, cfg.nx // px
+    small = cfg.scaled(py, px)
+    hs, Ts = synth.make_height(small, DEV), synth.make_target(small, DEV)
+    lambdas = cfg.lambdas if lambdas_idx is None else tuple(cfg.lambdas[i] for i in lambdas_idx)
+    n_refr = cfg.n_refr[:len(lambdas)]
+    # the oracle works on the small grid with the small grid's pitch: same frequencies on bins R k
+    Ir, Lr, gr = oracle_l2(small, hs, Ts, lambdas, n_refr)
+    h, T = synth.tile_plane(hs, ry, rx), synth.tile_plane(Ts, ry, rx)
+    write_i = cfg.write_intensity
+    flags = dop.DOP_WRITE_INTENSITY if write_i else 0
+    plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, lambdas, n_refr, cfg.z, dop.DOP_LOSS_L2, cfg.sigma_px, flags, DEV)
+    inten = torch.empty((len(lambdas), cfg.ny, cfg.nx), dtype=torch.float32, device=DEV) if write_i else None
+    grad = torch.empty_like(h)
+    loss = torch.zeros(1, dtype=torch.float64, device=DEV)
+    plan.fwd(h, T, inten, loss)
+    plan.adj(h, None, grad)
+    torch.cuda.synchronize()
+    plan.close()
+    assert abs(float(loss.item()) - Lr) <= TOL_LOSS * abs(Lr)
+    # every tile of the big result must equal the small one; compare all tiles on the device, one tile-row at a time
+    def cmp_tiles(big, small_np, what):
+        sm = torch.from_numpy(np.ascontiguousarray(small_np)).to(DEV)
+        num = 0.0
+        peak = 0.0
+        for iy in range(ry):
+            blk = big[iy * py:(iy + 1) * py].view(py, rx, px).permute(1, 0, 2).double() - sm
+            num += float((blk ** 2).sum().item())
+            peak = max(peak, float(blk.abs().max().item()))
+            del blk
+        e2 = np.sqrt(num) / (float((sm ** 2).sum().sqrt().item()) * np.sqrt(ry * rx))
+        ep = peak / float(sm.abs().max().item())
+        assert e2 <= TOL_L2 and ep <= TOL_PEAK, f"{name} tiled {what}: rel-L2 {e2:.3e}, max-abs/peak {ep:.3e}"
+
+    cmp_tiles(grad, gr / (ry * rx), "dL/dh")
+    if inten is not None:
+        for l in range(len(lambdas)):
+            cmp_tiles(inten[l], Ir[l], "I")
+
+
+def test_C2_full_size_tiled():
+    tiled_case("C2", 1024, 2048)
+
+
+def test_C3_full_size_tiled_with_prefilter():
+    tiled_case("C3", 2048, 1024)
+
+
+def plane_wave_case(name, a, b, p, q, tau=0.25, nsamp=4096):
+    """Pin P-i at full size: h = (lambda/(n-1)) frac(a x/Nx + b y/Ny) makes u0 the DFT basis vector
+    (a,b), so u = H(a,b) u0, I = |H|^2, and with T = 1 - tau cos(theta) the gradient has the closed
+    form of SURVEY.md 8(c) P-i, evaluated in fp64 at sampled points."""
+    cfg = synth.CONFIGS[name]
+    ny, nx, lam, n, z, pitch = cfg.ny, cfg.nx, cfg.lambdas[0], cfg.n_refr[0], cfg.z, cfg.pitch
+    ys = torch.arange(ny, device=DEV, dtype=torch.int64)[:, None]
+    xs = torch.arange(nx, device=DEV, dtype=torch.int64)[None, :]
+    h = torch.empty((ny, nx), dtype=torch.float32, device=DEV)
+    T = torch.empty((ny, nx), dtype=torch.float32, device=DEV)
+    rows = max(1, (1 << 26) // nx)
+    for y0 in range(0, ny, rows):
+        yy = ys[y0:y0 + rows]
+        # exact rational phase: (a x Ny + b y Nx) mod (Nx Ny) / (Nx Ny), in int64 then fp64
+        num = (a * xs * ny + b * yy * nx) % (nx * ny)
+        h[y0:y0 + rows] = ((lam / (n - 1)) * (num.double() / float(nx * ny))).float()
+        th = (p * xs * ny + q * yy * nx) % (nx * ny)
+        T[y0:y0 + rows] = (1.0 - tau * torch.cos(2 * np.pi * th.double() / float(nx * ny))).float()
+    flags = dop.DOP_WRITE_INTENSITY if cfg.write_intensity else 0
+    plan = dop.Plan(ny, nx, pitch, (lam,), (n,), z, dop.DOP_LOSS_L2, 0.0, flags, DEV)
+    inten = torch.empty((1, ny, nx), dtype=torch.float32, device=DEV) if flags else None
+    grad = torch.empty_like(h)
+    loss = torch.zeros(1, dtype=torch.float64, device=DEV)
+    plan.fwd(h, T, inten, loss)
+    plan.adj(h, None, grad)
+    torch.cuda.synchronize()
+    plan.close()
+
+    def H(ka, kb):
+        arg = 1 / lam ** 2 - (ka / (nx * pitch)) ** 2 - (kb / (ny * pitch)) ** 2
+        return np.exp(2j * np.pi * z * np.sqrt(arg)) if arg >= 0 else 0.0
+
+    H0, Hp, Hm = H(a, b), H(a + p, b + q), H(a - p, b - q)
+    assert abs(H0) == 1.0 and abs(Hp) == 1.0 and abs(Hm) == 1.0
+    rng = np.random.default_rng(11)
+    sy, sx = rng.integers(0, ny, nsamp), rng.integers(0, nx, nsamp)
+    th = 2 * np.pi * (((p * sx * ny + q * sy * nx) % (nx * ny)) / float(nx * ny))
+    # the fp32-rounded h the GPU saw defines u0; use it for the closed form's u0 phase
+    hs = h[torch.from_numpy(sy).to(DEV), torch.from_numpy(sx).to(DEV)].double().cpu().numpy()
+    N = float(nx * ny)
+    gref = (2 * np.pi * (n - 1) / lam) * (2 * tau / N) * np.imag(
+        H0 * (np.conj(Hp) * np.exp(1j * th) + np.conj(Hm) * np.exp(-1j * th)))
+    gs = grad[torch.from_numpy(sy).to(DEV), torch.from_numpy(sx).to(DEV)].double().cpu().numpy()
+    # loss: I == 1 exactly, so L = mean (tau cos)^2 = tau^2/2
+    assert abs(float(loss.item()) - tau * tau / 2) <= 2e-5 * tau * tau / 2
+    e2 = np.linalg.norm(gs - gref) / np.linalg.norm(gref)
+    ep = np.abs(gs - gref).max() / np.abs(gref).max()
+    # the closed form assumes h exact; fp32 storage of h perturbs the phase by ~4e-7 rad, below the bar
+    assert e2 <= 2e-5 and ep <= TOL_PEAK, f"{name} plane-wave dL/dh: {e2:.3e} {ep:.3e}"
+    assert hs.min() >= 0
+    if inten is not None:
+        Is = inten[0][torch.from_numpy(sy).to(DEV), torch.from_numpy(sx).to(DEV)].cpu().numpy()
+        assert np.abs(Is - 1.0).max() <= 1e-4
+
+
+def test_C2_full_size_plane_wave_closed_form():
+    plane_wave_case("C2", 1203, -877, 345, 210)
+
+
+HUGE = pytest.mark.skipif(os.environ.get("DOP_SKIP_HUGE") == "1" or not torch.cuda.is_available()
+                          or torch.cuda.get_device_properties(0).total_memory < 150e9,
+                          reason="needs ~130 GB of device memory")
+
+
+@HUGE
+def test_C4_full_size_tiled():
+    tiled_case("C4", 2048, 4096)
+
+
+@HUGE
+def test_C5_full_size_tiled():
+    tiled_case("C5", 3072, 2048)
+
+
+@HUGE
+def test_C5_full_size_plane_wave_closed_form():
+    plane_wave_case("C5", 5001, -3 * 2111, 1234, 3 * 777)
