@@ -15,8 +15,7 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
 
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream)
 {
-    static const bool force_generic = std::getenv("DOP_FORCE_GENERIC") != nullptr;
-    if (!force_generic) {
+    {
         bool handled = false;
         cudaError_t e = launch_tile_pass_pow2(p, stream, &handled);
         if (handled) return e;
@@ -58,6 +57,9 @@ dop_status ensure_device(dop_plan* p)
     for (int a = 0; a < 2; ++a)
         for (Digit& g : p->ax[a].dig)
             if (g.has_twb) { g.twb_off = off; off += align256(g.twb.size() * sizeof(float2)); }
+    for (int a = 0; a < 2; ++a)
+        for (Digit& g : p->ax[a].dig)
+            if (g.fast) { g.twg_off = off; off += align256(g.twg.size() * sizeof(float2)); }
     for (int a = 0; a < 2; ++a) {
         p->pi_off[a].resize(p->ax[a].dig.size());
         for (size_t j = 0; j < p->ax[a].dig.size(); ++j) { p->pi_off[a][j] = off; off += align256(p->ax[a].dig[j].pi.size() * sizeof(int)); }
@@ -77,6 +79,9 @@ dop_status ensure_device(dop_plan* p)
     for (int a = 0; a < 2; ++a)
         for (Digit& g : p->ax[a].dig)
             if (g.has_twb) up(g.twb_off, g.twb.data(), g.twb.size() * sizeof(float2));
+    for (int a = 0; a < 2; ++a)
+        for (Digit& g : p->ax[a].dig)
+            if (g.fast) up(g.twg_off, g.twg.data(), g.twg.size() * sizeof(float2));
     for (int a = 0; a < 2; ++a)
         for (size_t j = 0; j < p->ax[a].dig.size(); ++j) up(p->pi_off[a][j], p->ax[a].dig[j].pi.data(), p->ax[a].dig[j].pi.size() * sizeof(int));
     for (int a = 0; a < 2; ++a) {
@@ -104,6 +109,8 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.wL = (const float2*)(arena + p->wl_off[(size_t)g.wl_index]);
     d.pi = (const int*)(arena + p->pi_off[t.axis][(size_t)t.digit]);
     d.tw_b = g.has_twb ? (const float2*)(arena + g.twb_off) : nullptr;
+    d.twb_n = g.L * g.st;
+    d.tw_g = g.fast ? (const float2*)(arena + g.twg_off) : nullptr;
     d.load_op = t.load_op;
     d.mid_op = t.mid_op;
     d.store_op = t.store_op;

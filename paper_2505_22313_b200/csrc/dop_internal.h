@@ -66,6 +66,8 @@ struct PassDesc {
     const float2* wL;   // [L]  W_L^p = exp(-2 pi i p / L)
     const int* pi;      // [L]  slot within digit -> output index k_j
     const float2* tw_b; // [N_j] boundary twiddles W_{N_j}^p, or nullptr
+    long long twb_n;    // N_j = L_j st_j
+    const float2* tw_g; // group twiddles of the register-blocked schedule (fft_regs.cuh), or nullptr
     int r_from;         // 0: r_j = c (x digit), 1: r_j = m (y digit)
     // ---- pointwise ops
     int load_op, mid_op, store_op;
@@ -90,6 +92,10 @@ struct PassDesc {
 };
 
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream);
+// register-blocked power-of-two fast path (kernels_pow2.cu)
+bool pow2_supported(long long L, bool col_type);
+int pow2_lines(long long L, bool col_type);
+std::vector<float2> pow2_group_twiddles(long long L);
 cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
                                cudaStream_t stream);
 
@@ -103,7 +109,10 @@ struct Digit {
     int wl_index = -1;            // which W_L table
     bool has_twb = false;
     std::vector<float2> twb;      // W_{L st}^p, p < L st
-    size_t twb_off = 0;           // offset (float2) into the device twiddle arena
+    size_t twb_off = 0;           // byte offset into the device arena
+    bool fast = false;            // handled by the register-blocked pow2 kernels
+    std::vector<float2> twg;      // their group twiddles
+    size_t twg_off = 0;
 };
 
 struct Axis {
@@ -136,6 +145,7 @@ struct dop_plan {
     std::vector<long long> wl_len;
     std::vector<size_t> wl_off;
     int tile_pts = 4096;
+    bool force_generic = false; // DOP_FORCE_GENERIC at plan creation: generic kernel for every pass
     // schedules for one lambda
     std::vector<dop::PassTmpl> fwd, adj, pre; // pre = Gaussian pre-filter (real -> real)
     long long loss_tiles = 0;                 // CTAs of the MID_LOSS pass

@@ -1,0 +1,247 @@
+// fft_regs.cuh -- register-blocked power-of-two line FFT for one CTA tile (sm_100a).
+//
+// Same mathematics and the same slot order as the generic in-place kernel (kernels_generic.cu):
+// in-place decimation in frequency over the radix list (4, 4, ..., 4[, 2]) of a digit of length
+// L = 2^p, inverse = exact mirror (decimation in time, conjugate twiddles).  What differs is where
+// the data lives: every thread keeps P = 16 points in registers and runs up to two radix-4
+// sub-steps (one radix-16 "group") without touching memory; groups exchange data through shared
+// memory (one 64-bit store + one 64-bit load per point), and the first / last group load from and
+// store to global memory directly from registers.  See DESIGN.md "Kernels".
+//
+//   group g:  block length n_g, radix R_g = RA*RB (RA in {2,4}, RB in {1,2,4}), m_g = n_g / R_g
+//   butterfly id bf in [0, L/R_g):  b = bf / m_g,  j = bf % m_g,  slots  b n_g + j + c m_g, c < R_g
+//   register c = ca RB + cb  <->  after the group register c' = ca' RB + cb' holds the output of
+//   frequency k = ca' + RA cb' (digit-reversed within the group), times W_{n_g}^{j k}.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace dop {
+namespace fx {
+
+constexpr int P = 16; // points per thread
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{
+    return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) // a * conj(b)
+{
+    return make_float2(fmaf(a.y, b.y, a.x * b.x), fmaf(-a.x, b.y, a.y * b.x));
+}
+
+// ---- compile-time schedule of a digit of length L ---------------------------------------------
+__host__ __device__ constexpr int ilog2(int x) { return x <= 1 ? 0 : 1 + ilog2(x >> 1); }
+
+template <int L>
+struct Sched {
+    static constexpr int LG = ilog2(L);
+    static constexpr int N4 = LG / 2;       // radix-4 sub-steps
+    static constexpr int N2 = LG & 1;       // trailing radix-2 sub-step
+    static constexpr int NFULL = N4 / 2;    // radix-16 groups
+    static constexpr int REM4 = N4 & 1;
+    static constexpr int RLAST = (REM4 ? 4 : 1) * (N2 ? 2 : 1); // 1 = no remainder group
+    static constexpr int NG = NFULL + (RLAST > 1 ? 1 : 0);
+    __host__ __device__ static constexpr int radix(int g) { return g < NFULL ? 16 : RLAST; }
+    __host__ __device__ static constexpr int block(int g) { return g == 0 ? L : block(g - 1) / radix(g - 1); } // n_g
+    __host__ __device__ static constexpr int twoff(int g) // offset (float2) of group g's twiddle table
+    {
+        return g == 0 ? 0 : twoff(g - 1) + (radix(g - 1) - 1) * (block(g - 1) / radix(g - 1));
+    }
+    static constexpr int TWSIZE = twoff(NG); // the last group's (m = 1) entries are never read
+};
+
+// ---- radix-2 / radix-4 butterflies on registers -----------------------------------------------
+template <int DIR>
+__device__ __forceinline__ void bf2(float2& a, float2& b)
+{
+    float2 t = a;
+    a = make_float2(t.x + b.x, t.y + b.y);
+    b = make_float2(t.x - b.x, t.y - b.y);
+}
+template <int DIR>
+__device__ __forceinline__ void bf4(float2& a, float2& b, float2& c, float2& d)
+{
+    float2 s0 = make_float2(a.x + c.x, a.y + c.y), s1 = make_float2(a.x - c.x, a.y - c.y);
+    float2 s2 = make_float2(b.x + d.x, b.y + d.y), s3 = make_float2(b.x - d.x, b.y - d.y);
+    a = make_float2(s0.x + s2.x, s0.y + s2.y);
+    c = make_float2(s0.x - s2.x, s0.y - s2.y);
+    if (DIR > 0) { // b = s1 - i s3, d = s1 + i s3
+        b = make_float2(s1.x + s3.y, s1.y - s3.x);
+        d = make_float2(s1.x - s3.y, s1.y + s3.x);
+    } else {
+        b = make_float2(s1.x - s3.y, s1.y + s3.x);
+        d = make_float2(s1.x + s3.y, s1.y - s3.x);
+    }
+}
+
+// v *= W_16^{E} (DIR > 0) or its conjugate (DIR < 0), E a compile-time exponent
+template <int E, int DIR>
+__device__ __forceinline__ void mul_w16(float2& v)
+{
+    constexpr int e = ((E % 16) + 16) % 16;
+    constexpr float C1 = 0.92387953251128675613f, S1 = 0.38268343236508977173f, H = 0.70710678118654752440f;
+    // W16^e = cos(2 pi e/16) - i sin(2 pi e/16)
+    constexpr float co[16] = {1.f, C1, H, S1, 0.f, -S1, -H, -C1, -1.f, -C1, -H, -S1, 0.f, S1, H, C1};
+    constexpr float si[16] = {0.f, S1, H, C1, 1.f, C1, H, S1, 0.f, -S1, -H, -C1, -1.f, -C1, -H, -S1};
+    if (e == 0) return;
+    const float c = co[e], s = (DIR > 0) ? -si[e] : si[e]; // multiply by (c + i s)
+    if (e == 4 || e == 12) {
+        v = make_float2(-s * v.y, s * v.x);
+    } else if (e == 8) {
+        v = make_float2(-v.x, -v.y);
+    } else {
+        v = make_float2(fmaf(-s, v.y, c * v.x), fmaf(s, v.x, c * v.y));
+    }
+}
+
+// One group butterfly on R = RA*RB registers v[0], v[ST], ..., v[(R-1) ST] (ST = register stride).
+template <int RA, int RB, int DIR, int ST>
+__device__ __forceinline__ void group(float2* v)
+{
+    constexpr int R = RA * RB;
+    if (DIR > 0) {
+#pragma unroll
+        for (int cb = 0; cb < RB; ++cb) {
+            if (RA == 4) bf4<DIR>(v[(0 * RB + cb) * ST], v[(1 * RB + cb) * ST], v[(2 * RB + cb) * ST], v[(3 * RB + cb) * ST]);
+            else bf2<DIR>(v[(0 * RB + cb) * ST], v[(1 * RB + cb) * ST]);
+        }
+        if (RB > 1) {
+            // internal twiddles W_R^{cb ca'} = W_16^{cb ca' 16/R}
+#define DOP_TW(CA, CB) mul_w16<(CA) * (CB) * (16 / R), DIR>(v[((CA) * RB + (CB)) * ST])
+            if (RA == 4 && RB == 4) {
+                DOP_TW(1, 1); DOP_TW(1, 2); DOP_TW(1, 3);
+                DOP_TW(2, 1); DOP_TW(2, 2); DOP_TW(2, 3);
+                DOP_TW(3, 1); DOP_TW(3, 2); DOP_TW(3, 3);
+            } else if (RA == 4 && RB == 2) {
+                DOP_TW(1, 1); DOP_TW(2, 1); DOP_TW(3, 1);
+            }
+#pragma unroll
+            for (int ca = 0; ca < RA; ++ca) {
+                if (RB == 4) bf4<DIR>(v[(ca * RB + 0) * ST], v[(ca * RB + 1) * ST], v[(ca * RB + 2) * ST], v[(ca * RB + 3) * ST]);
+                else bf2<DIR>(v[(ca * RB + 0) * ST], v[(ca * RB + 1) * ST]);
+            }
+        }
+    } else {
+        if (RB > 1) {
+#pragma unroll
+            for (int ca = 0; ca < RA; ++ca) {
+                if (RB == 4) bf4<DIR>(v[(ca * RB + 0) * ST], v[(ca * RB + 1) * ST], v[(ca * RB + 2) * ST], v[(ca * RB + 3) * ST]);
+                else bf2<DIR>(v[(ca * RB + 0) * ST], v[(ca * RB + 1) * ST]);
+            }
+            if (RA == 4 && RB == 4) {
+                DOP_TW(1, 1); DOP_TW(1, 2); DOP_TW(1, 3);
+                DOP_TW(2, 1); DOP_TW(2, 2); DOP_TW(2, 3);
+                DOP_TW(3, 1); DOP_TW(3, 2); DOP_TW(3, 3);
+            } else if (RA == 4 && RB == 2) {
+                DOP_TW(1, 1); DOP_TW(2, 1); DOP_TW(3, 1);
+            }
+#undef DOP_TW
+        }
+#pragma unroll
+        for (int cb = 0; cb < RB; ++cb) {
+            if (RA == 4) bf4<DIR>(v[(0 * RB + cb) * ST], v[(1 * RB + cb) * ST], v[(2 * RB + cb) * ST], v[(3 * RB + cb) * ST]);
+            else bf2<DIR>(v[(0 * RB + cb) * ST], v[(1 * RB + cb) * ST]);
+        }
+    }
+}
+
+template <int R> struct Split;
+template <> struct Split<16> { static constexpr int RA = 4, RB = 4; };
+template <> struct Split<8> { static constexpr int RA = 4, RB = 2; };
+template <> struct Split<4> { static constexpr int RA = 4, RB = 1; };
+template <> struct Split<2> { static constexpr int RA = 2, RB = 1; };
+
+// frequency index (within the group) held by register c' after a forward group
+template <int R>
+__host__ __device__ constexpr int group_freq(int c)
+{
+    return (c / Split<R>::RB) + Split<R>::RA * (c % Split<R>::RB);
+}
+
+// ---- tile-level engine --------------------------------------------------------------------------
+// Shared-memory layout of one tile.
+//   COL = true : NB = 16 adjacent lines; element (slot, col) at slot*16 + col (conflict-free).
+//   COL = false: one line; slot s at s + 2*(s >> 5) (two pad elements per 32 keep every access
+//                pattern of the schedule conflict-free and 16-byte alignment of even slots).
+template <int L, bool COL>
+struct Tile {
+    using S = Sched<L>;
+    static constexpr int T = L / P;                                   // threads per line
+    static constexpr int LINE_ELEMS = COL ? L * 16 : L + 2 * (L / 32); // float2 per tile (COL) / line (row)
+
+    __device__ static __forceinline__ int addr(int slot, int off)
+    {
+        return COL ? (slot << 4) + off : slot + ((slot >> 5) << 1) + off;
+    }
+    // slot of register i in the layout of group G
+    template <int G>
+    __device__ static __forceinline__ int slot(int tt, int i)
+    {
+        constexpr int R = S::radix(G), m = S::block(G) / R;
+        const int u = i / R, c = i % R;
+        const int bf = tt + u * T;
+        return (bf & ~(m - 1)) * R + (bf & (m - 1)) + c * m;
+    }
+    template <int G>
+    __device__ static __forceinline__ void to_smem(const float2* v, float2* s, int tt, int off)
+    {
+#pragma unroll
+        for (int i = 0; i < P; ++i) s[addr(slot<G>(tt, i), off)] = v[i];
+    }
+    template <int G>
+    __device__ static __forceinline__ void from_smem(float2* v, const float2* s, int tt, int off)
+    {
+#pragma unroll
+        for (int i = 0; i < P; ++i) v[i] = s[addr(slot<G>(tt, i), off)];
+    }
+    template <int G, int DIR>
+    __device__ static __forceinline__ void butterflies(float2* v, int tt, const float2* __restrict__ tw)
+    {
+        constexpr int R = S::radix(G), m = S::block(G) / R;
+#pragma unroll
+        for (int u = 0; u < P / R; ++u) {
+            float2* w = v + u * R;
+            const int j = (tt + u * T) & (m - 1);
+            if (DIR < 0 && m > 1) {
+#pragma unroll
+                for (int c = 1; c < R; ++c)
+                    w[c] = cmulc(w[c], __ldg(tw + S::twoff(G) + (group_freq<R>(c) - 1) * m + j));
+            }
+            group<Split<R>::RA, Split<R>::RB, DIR, 1>(w);
+            if (DIR > 0 && m > 1) {
+#pragma unroll
+                for (int c = 1; c < R; ++c)
+                    w[c] = cmul(w[c], __ldg(tw + S::twoff(G) + (group_freq<R>(c) - 1) * m + j));
+            }
+        }
+    }
+    // forward: v in the layout of group 0  ->  v in the layout of the last group
+    template <int G = 0>
+    __device__ static __forceinline__ void forward(float2* v, float2* s, int tt, int off, const float2* __restrict__ tw)
+    {
+        butterflies<G, +1>(v, tt, tw);
+        if constexpr (G + 1 < S::NG) {
+            to_smem<G>(v, s, tt, off);
+            __syncthreads();
+            from_smem<G + 1>(v, s, tt, off);
+            __syncthreads();
+            forward<G + 1>(v, s, tt, off, tw);
+        }
+    }
+    // inverse (unnormalised): v in the layout of the last group  ->  layout of group 0
+    template <int G = S::NG - 1>
+    __device__ static __forceinline__ void inverse(float2* v, float2* s, int tt, int off, const float2* __restrict__ tw)
+    {
+        butterflies<G, -1>(v, tt, tw);
+        if constexpr (G > 0) {
+            to_smem<G>(v, s, tt, off);
+            __syncthreads();
+            from_smem<G - 1>(v, s, tt, off);
+            __syncthreads();
+            inverse<G - 1>(v, s, tt, off, tw);
+        }
+    }
+};
+
+} // namespace fx
+} // namespace dop

@@ -136,6 +136,11 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         d.wl_index = wl_table_index(p, d.L);
         d.has_twb = (j + 1 < Ls.size());
         if (d.has_twb) d.twb = twiddle_table(d.L * d.st);
+        // column-type unless it is the last x digit
+        const bool col_type = !(a == 0 && d.st == 1);
+        const long long lines = col_type ? (a == 0 ? d.st : p->desc.nx) : p->desc.ny * (N / d.L);
+        d.fast = !p->force_generic && pow2_supported(d.L, col_type) && lines % pow2_lines(d.L, col_type) == 0;
+        if (d.fast) d.twg = pow2_group_twiddles(d.L);
     }
     // slot -> true frequency index:  k = sum_j pi_j(p_j) (L_0 .. L_{j-1})
     ax.kslot.resize((size_t)N);
@@ -214,6 +219,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
     d->n_radix = (int)g.radix.size();
     for (int i = 0; i < d->n_radix; ++i) d->radix[i] = g.radix[(size_t)i];
     long long nl_target = std::max<long long>(1, p->tile_pts / L);
+    const bool fast = g.fast;
     d->row_o = d->row_m = d->row_i = 0;
     if (axis == 0 && st == 1) { // last x digit: row-type, lines are contiguous runs of L
         d->col_type = 0;
@@ -222,7 +228,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
         d->SCc = L;
         d->n_m = 1; d->SM = 0; d->n_o = 1; d->SO = 0;
         d->r_from = 0;
-        d->nl = (int)std::min<long long>(nl_target, d->NC);
+        d->nl = fast ? pow2_lines(L, false) : (int)std::min<long long>(nl_target, d->NC);
     } else if (axis == 0) { // higher x digit: lines r..r+nl-1 adjacent, elements st apart
         d->col_type = 1;
         d->es = st;
@@ -230,7 +236,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
         d->n_m = nx / (L * st); d->SM = L * st;
         d->n_o = ny; d->SO = nx;
         d->r_from = 0;
-        d->nl = (int)std::min<long long>(std::max<long long>(nl_target, 16), st);
+        d->nl = fast ? 16 : (int)std::min<long long>(std::max<long long>(nl_target, 16), st);
     } else { // y digit: lines are adjacent columns, elements st rows apart
         d->col_type = 1;
         d->es = st * nx;
@@ -239,7 +245,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
         d->n_o = ny / (L * st); d->SO = L * st * nx;
         d->r_from = 1;
         d->row_o = L * st; d->row_m = 1; d->row_i = st;
-        d->nl = (int)std::min<long long>(std::max<long long>(nl_target, 16), nx);
+        d->nl = fast ? 16 : (int)std::min<long long>(std::max<long long>(nl_target, 16), nx);
     }
     d->n_cgroups = (d->NC + d->nl - 1) / d->nl;
     d->smem_bytes = (int)((long long)d->nl * L * (long long)sizeof(float2));
@@ -250,6 +256,7 @@ dop_status build_plan(dop_plan* p)
 {
     const dop_plan_desc& d = p->desc;
     if (!is_23_smooth(d.nx) || !is_23_smooth(d.ny)) return DOP_ERR_UNSUPPORTED_SIZE;
+    p->force_generic = std::getenv("DOP_FORCE_GENERIC") != nullptr;
     if (const char* e = std::getenv("DOP_TILE_PTS")) {
         int v = std::atoi(e);
         if (v >= 256 && v <= 16384) p->tile_pts = v;
@@ -300,7 +307,7 @@ std::string describe_plan(const dop_plan* p)
             PassDesc g{};
             tile_geometry(p, t.axis, t.digit, &g);
             os << tag << " " << (t.axis == 0 ? "x" : "y") << t.digit << " L=" << g.L << " tile=" << g.nl << "x" << g.L
-               << (g.col_type ? " col" : " row") << " ctas=" << g.n_cgroups * g.n_m * g.n_o
+               << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? " pow2" : " generic") << " ctas=" << g.n_cgroups * g.n_m * g.n_o
                << " smem=" << g.smem_bytes << " B/pt=" << t.bytes_per_point << " [" << t.name << "]\n";
             total += t.bytes_per_point;
         }
