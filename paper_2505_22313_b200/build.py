@@ -2,9 +2,13 @@
 
 In-tree on purpose: the .so travels to the GPU box with the repo snapshot and is what the tests,
 bench.py and __graft_entry__ load through ctypes.  nvcc cross-compiles without a GPU.
+The register-blocked kernels are instantiated per (tile type, digit length) in separate objects
+(pow2_inst.cu, once per entry of POW2_INST) so that they compile in parallel.
 """
 from __future__ import annotations
 
+import concurrent.futures
+import hashlib
 import os
 import subprocess
 import sys
@@ -12,11 +16,15 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdop.so")
+OBJDIR = os.path.join(HERE, "build")
 SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu"]
-HEADERS = ["dop_internal.h", os.path.join("..", "..", "include", "dop.h")]
+# (column-type?, digit length) -- must match the DOP_DECL list in kernels_pow2.cu
+POW2_INST = [(1, L) for L in (16, 32, 64, 128, 256, 512)] + \
+            [(0, L) for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192)]
+HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", os.path.join("..", "..", "include", "dop.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC",
 ]
 
 
@@ -27,23 +35,60 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _units():
+    """(object path, source path, extra flags) of every translation unit."""
+    units = [(os.path.join(OBJDIR, s.replace(".cu", ".o")), os.path.join(CSRC, s), []) for s in SOURCES]
+    for col, L in POW2_INST:
+        units.append((os.path.join(OBJDIR, f"pow2_{'col' if col else 'row'}_{L}.o"),
+                      os.path.join(CSRC, "pow2_inst.cu"), [f"-DDOP_INST_COL={col}", f"-DDOP_INST_L={L}"]))
+    return units
+
+
+def _dep_stamp() -> str:
+    h = hashlib.sha256()
+    for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS + ["pow2_inst.cu"]] + [os.path.abspath(__file__)]:
+        with open(d, "rb") as f:
+            h.update(f.read())
+    h.update(" ".join(NVCC_FLAGS).encode())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    stamp = os.path.join(OBJDIR, "stamp")
+    if not os.path.exists(LIB) or not os.path.exists(stamp):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(stamp) as f:
+        return f.read().strip() != _dep_stamp()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile if libdop.so is missing or older than its sources; return its path."""
+    """Compile if libdop.so is missing or its sources changed; return its path."""
     if not force and not _stale():
         return LIB
+    os.makedirs(OBJDIR, exist_ok=True)
+    nvcc = _nvcc()
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(u):
+        obj, src, flags = u
+        r = subprocess.run([nvcc] + NVCC_FLAGS + extra + flags + ["-c", src, "-o", obj],
+                           capture_output=True, text=True)
+        return u, r
+
+    units = _units()
+    workers = max(1, min(len(units), os.cpu_count() or 4))
+    with concurrent.futures.ThreadPoolExecutor(workers) as ex:
+        for u, r in ex.map(compile_one, units):
+            if verbose or r.returncode != 0:
+                sys.stderr.write(f"== {os.path.basename(u[0])}\n{r.stdout}{r.stderr}")
+            if r.returncode != 0:
+                raise RuntimeError(f"nvcc failed for {u[0]}")
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.run(cmd, check=True)
+    subprocess.run([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a",
+                    "-o", tmp] + [u[0] for u in units], check=True)
     os.replace(tmp, LIB)
+    with open(os.path.join(OBJDIR, "stamp"), "w") as f:
+        f.write(_dep_stamp())
     return LIB
 
 

@@ -60,6 +60,9 @@ dop_status ensure_device(dop_plan* p)
     for (int a = 0; a < 2; ++a)
         for (Digit& g : p->ax[a].dig)
             if (g.fast) { g.twg_off = off; off += align256(g.twg.size() * sizeof(float2)); }
+    for (int a = 0; a < 2; ++a)
+        for (Digit& g : p->ax[a].dig)
+            if (!g.twb2.empty()) { g.twb2_off = off; off += align256(g.twb2.size() * sizeof(float2)); }
     for (int a = 0; a < 2; ++a) {
         p->pi_off[a].resize(p->ax[a].dig.size());
         for (size_t j = 0; j < p->ax[a].dig.size(); ++j) { p->pi_off[a][j] = off; off += align256(p->ax[a].dig[j].pi.size() * sizeof(int)); }
@@ -82,6 +85,9 @@ dop_status ensure_device(dop_plan* p)
     for (int a = 0; a < 2; ++a)
         for (Digit& g : p->ax[a].dig)
             if (g.fast) up(g.twg_off, g.twg.data(), g.twg.size() * sizeof(float2));
+    for (int a = 0; a < 2; ++a)
+        for (Digit& g : p->ax[a].dig)
+            if (!g.twb2.empty()) up(g.twb2_off, g.twb2.data(), g.twb2.size() * sizeof(float2));
     for (int a = 0; a < 2; ++a)
         for (size_t j = 0; j < p->ax[a].dig.size(); ++j) up(p->pi_off[a][j], p->ax[a].dig[j].pi.data(), p->ax[a].dig[j].pi.size() * sizeof(int));
     for (int a = 0; a < 2; ++a) {
@@ -109,6 +115,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.wL = (const float2*)(arena + p->wl_off[(size_t)g.wl_index]);
     d.pi = (const int*)(arena + p->pi_off[t.axis][(size_t)t.digit]);
     d.tw_b = g.has_twb ? (const float2*)(arena + g.twb_off) : nullptr;
+    d.tw_b2 = g.twb2.empty() ? nullptr : (const float2*)(arena + g.twb2_off);
     d.twb_n = g.L * g.st;
     d.tw_g = g.fast ? (const float2*)(arena + g.twg_off) : nullptr;
     d.load_op = t.load_op;
@@ -170,16 +177,91 @@ void prof_end(dop_plan* p, long long slot, cudaStream_t st)
     if (slot >= 0) cudaEventRecord(p->ev_stop[(size_t)slot], st);
 }
 
+long long gcdll(long long a, long long b) { while (b) { long long t = a % b; a = b; b = t; } return a; }
+long long lcmll(long long a, long long b) { return a / gcdll(a, b) * b; }
+
+std::string pass_label(const char* tag, const PassTmpl& t)
+{
+    return std::string(tag) + ":" + (t.axis == 0 ? "x" : "y") + std::to_string(t.digit) + ":" + t.name;
+}
+
+// One segment = consecutive passes along the same axis.  Its passes exchange data only inside
+// independent groups (y passes: inside a column group; x passes: inside a row), so the segment
+// is run slab by slab -- a slab being a set of whole groups of about slab_bytes -- and every pass
+// after the first finds its input in L2.
+dop_status run_segment(dop_plan* p, const std::vector<PassTmpl>& sched, size_t b, size_t e, int lam,
+                       const Buffers& bufs, char* ws, cudaStream_t st, const char* tag)
+{
+    const long long nx = p->desc.nx, ny = p->desc.ny;
+    const int axis = sched[b].axis;
+    std::vector<PassDesc> d;
+    for (size_t i = b; i < e; ++i) d.push_back(resolve(p, sched[i], lam, bufs, ws));
+    // slab unit (columns for y segments, rows for x segments) and slab size
+    long long unit = 1, total = axis == 1 ? nx : ny, per = total;
+    const bool slabbed = p->slab_bytes > 0 && e - b >= 2;
+    if (slabbed) {
+        for (const PassDesc& q : d) {
+            if (axis == 1) unit = lcmll(unit, q.nl);
+            else if (!q.col_type) {
+                const long long lpr = nx / q.L; // lines per row
+                if (q.nl > lpr) unit = lcmll(unit, (q.nl + lpr - 1) / lpr);
+            }
+        }
+        const long long group_bytes = (axis == 1 ? ny : nx) * (long long)sizeof(float2);
+        per = p->slab_bytes / group_bytes / unit * unit;
+        if (per < unit) per = unit;
+        if (per > total) per = total;
+    }
+    if (!slabbed || per >= total) { // whole-array launches, one profiling slot per launch
+        for (size_t i = b; i < e; ++i) {
+            long long slot = prof_begin(p, pass_label(tag, sched[i]), sched[i].bytes_per_point, st);
+            cudaError_t er = launch_tile_pass(d[i - b], st);
+            prof_end(p, slot, st);
+            if (er != cudaSuccess) return DOP_ERR_CUDA;
+        }
+        return DOP_OK;
+    }
+    std::string name = std::string(tag) + ":" + (axis == 0 ? "x" : "y") + "-seg[";
+    double dram = sched[b].rd + sched[e - 1].wr;
+    for (size_t i = b; i < e; ++i) {
+        name += (i > b ? " | " : "") + sched[i].name;
+        dram += sched[i].side;
+    }
+    name += "]";
+    long long slot = prof_begin(p, name, dram, st);
+    for (long long g0 = 0; g0 < total; g0 += per) {
+        const long long g1 = g0 + per < total ? g0 + per : total;
+        for (PassDesc q : d) {
+            if (axis == 1) { // columns [g0, g1)
+                q.cg0 = g0 / q.nl;
+                q.n_cgroups = (g1 - g0 + q.nl - 1) / q.nl;
+            } else if (q.col_type) { // rows [g0, g1)
+                q.tile0 = g0 * q.n_m * q.n_cgroups;
+                q.o0 = g0;
+                q.n_o = g1 - g0;
+            } else {
+                const long long lpr = nx / q.L;
+                q.cg0 = g0 * lpr / q.nl;
+                q.n_cgroups = ((g1 - g0) * lpr + q.nl - 1) / q.nl;
+                q.tile0 = q.cg0;
+            }
+            if (launch_tile_pass(q, st) != cudaSuccess) return DOP_ERR_CUDA;
+        }
+    }
+    prof_end(p, slot, st);
+    return DOP_OK;
+}
+
 dop_status run(dop_plan* p, const std::vector<PassTmpl>& sched, int lam, const Buffers& b, char* ws,
                cudaStream_t st, const char* tag)
 {
-    for (const PassTmpl& t : sched) {
-        PassDesc d = resolve(p, t, lam, b, ws);
-        long long slot = prof_begin(p, std::string(tag) + ":" + (t.axis == 0 ? "x" : "y") + std::to_string(t.digit) + ":" + t.name,
-                                    t.bytes_per_point, st);
-        cudaError_t e = launch_tile_pass(d, st);
-        prof_end(p, slot, st);
-        if (e != cudaSuccess) return DOP_ERR_CUDA;
+    size_t i = 0;
+    while (i < sched.size()) {
+        size_t j = i + 1;
+        while (j < sched.size() && sched[j].axis == sched[i].axis) ++j;
+        dop_status s = run_segment(p, sched, i, j, lam, b, ws, st, tag);
+        if (s != DOP_OK) return s;
+        i = j;
     }
     return DOP_OK;
 }

@@ -58,6 +58,9 @@ struct PassDesc {
     long long n_m, SM; // middle coordinate
     long long n_o, SO; // outer coordinate
     long long n_cgroups;
+    // ---- slab launch (a launch may cover only a range of column groups / outer indices)
+    long long cg0, o0; // added to the decoded cg / o
+    long long tile0;   // global tile index of this launch's first tile (loss partial slot)
     // ---- in-tile DFT
     int n_radix;
     int radix[kMaxRadixSteps];
@@ -66,6 +69,7 @@ struct PassDesc {
     const float2* wL;   // [L]  W_L^p = exp(-2 pi i p / L)
     const int* pi;      // [L]  slot within digit -> output index k_j
     const float2* tw_b; // [N_j] boundary twiddles W_{N_j}^p, or nullptr
+    const float2* tw_b2; // the same twiddles permuted for the pow2 kernels: y digits [r][slot], x digits [slot][r]
     long long twb_n;    // N_j = L_j st_j
     const float2* tw_g; // group twiddles of the register-blocked schedule (fft_regs.cuh), or nullptr
     int r_from;         // 0: r_j = c (x digit), 1: r_j = m (y digit)
@@ -113,6 +117,8 @@ struct Digit {
     bool fast = false;            // handled by the register-blocked pow2 kernels
     std::vector<float2> twg;      // their group twiddles
     size_t twg_off = 0;
+    std::vector<float2> twb2;     // boundary twiddles in the pow2 kernels' layout (fast digits with has_twb)
+    size_t twb2_off = 0;
 };
 
 struct Axis {
@@ -133,6 +139,7 @@ struct PassTmpl {
     int load_op, mid_op, store_op;
     std::string name;
     double bytes_per_point; // algorithmic HBM bytes per grid point of this launch
+    double rd, wr, side;    // its parts: main input read, main output written, side planes (T, I, h, grad)
 };
 
 } // namespace dop
@@ -145,6 +152,7 @@ struct dop_plan {
     std::vector<long long> wl_len;
     std::vector<size_t> wl_off;
     int tile_pts = 4096;
+    long long slab_bytes = 0;   // L2 slab size for multi-pass segments (0 = whole-array launches)
     bool force_generic = false; // DOP_FORCE_GENERIC at plan creation: generic kernel for every pass
     // schedules for one lambda
     std::vector<dop::PassTmpl> fwd, adj, pre; // pre = Gaussian pre-filter (real -> real)

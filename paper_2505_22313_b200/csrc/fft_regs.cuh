@@ -20,13 +20,45 @@ namespace fx {
 
 constexpr int P = 16; // points per thread
 
-__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+// ---- packed fp32x2 arithmetic (sm_100a FADD2 / FMUL2 / FFMA2) ----------------------------------
+// A complex64 value is a 64-bit register pair, so one complex add is ONE packed instruction and a
+// complex multiply is TWO (FMUL2 + FFMA2); the half-swap / per-half-negate operand modifiers of
+// the packed instructions (SASS .LO_HI / .NP, scalar broadcast R.F32) make the +-i rotations and
+// the (v.y,v.y) x (w.y,w.x) terms free.  The packed pipe retires 2 lanes per instruction at half
+// the issue rate: same flop/s as scalar FADD/FFMA, half the issue slots.
+__device__ __forceinline__ float2 add2(float2 a, float2 b)
 {
-    return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.x, b.y, a.y * b.x));
+    float2 r;
+    asm("{ .reg .b64 a,b,c; mov.b64 a,{%2,%3}; mov.b64 b,{%4,%5}; add.rn.f32x2 c,a,b; mov.b64 {%0,%1},c; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b)
+{
+    float2 r;
+    asm("{ .reg .b64 a,b,c; mov.b64 a,{%2,%3}; mov.b64 b,{%4,%5}; mul.rn.f32x2 c,a,b; mov.b64 {%0,%1},c; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
+{
+    float2 r;
+    asm("{ .reg .b64 a,b,c,d; mov.b64 a,{%2,%3}; mov.b64 b,{%4,%5}; mov.b64 c,{%6,%7}; fma.rn.f32x2 d,a,b,c; "
+        "mov.b64 {%0,%1},d; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return r;
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return add2(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return add2(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) // a * b
+{
+    const float2 t = mul2(make_float2(a.y, a.y), make_float2(b.y, b.x));
+    return fma2(make_float2(a.x, a.x), b, make_float2(-t.x, t.y));
 }
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b) // a * conj(b)
 {
-    return make_float2(fmaf(a.y, b.y, a.x * b.x), fmaf(-a.x, b.y, a.y * b.x));
+    const float2 t = mul2(make_float2(a.x, a.x), b);
+    return fma2(make_float2(a.y, a.y), make_float2(b.y, b.x), make_float2(t.x, -t.y));
 }
 
 // ---- compile-time schedule of a digit of length L ---------------------------------------------
@@ -54,23 +86,23 @@ struct Sched {
 template <int DIR>
 __device__ __forceinline__ void bf2(float2& a, float2& b)
 {
-    float2 t = a;
-    a = make_float2(t.x + b.x, t.y + b.y);
-    b = make_float2(t.x - b.x, t.y - b.y);
+    const float2 t = a;
+    a = cadd(t, b);
+    b = csub(t, b);
 }
 template <int DIR>
 __device__ __forceinline__ void bf4(float2& a, float2& b, float2& c, float2& d)
 {
-    float2 s0 = make_float2(a.x + c.x, a.y + c.y), s1 = make_float2(a.x - c.x, a.y - c.y);
-    float2 s2 = make_float2(b.x + d.x, b.y + d.y), s3 = make_float2(b.x - d.x, b.y - d.y);
-    a = make_float2(s0.x + s2.x, s0.y + s2.y);
-    c = make_float2(s0.x - s2.x, s0.y - s2.y);
+    const float2 s0 = cadd(a, c), s1 = csub(a, c), s2 = cadd(b, d), s3 = csub(b, d);
+    a = cadd(s0, s2);
+    c = csub(s0, s2);
+    const float2 r = make_float2(s3.y, -s3.x); // -i s3 (folded into the operand modifiers)
     if (DIR > 0) { // b = s1 - i s3, d = s1 + i s3
-        b = make_float2(s1.x + s3.y, s1.y - s3.x);
-        d = make_float2(s1.x - s3.y, s1.y + s3.x);
+        b = cadd(s1, r);
+        d = csub(s1, r);
     } else {
-        b = make_float2(s1.x - s3.y, s1.y + s3.x);
-        d = make_float2(s1.x + s3.y, s1.y - s3.x);
+        b = csub(s1, r);
+        d = cadd(s1, r);
     }
 }
 
@@ -85,12 +117,17 @@ __device__ __forceinline__ void mul_w16(float2& v)
     constexpr float si[16] = {0.f, S1, H, C1, 1.f, C1, H, S1, 0.f, -S1, -H, -C1, -1.f, -C1, -H, -S1};
     if (e == 0) return;
     const float c = co[e], s = (DIR > 0) ? -si[e] : si[e]; // multiply by (c + i s)
-    if (e == 4 || e == 12) {
-        v = make_float2(-s * v.y, s * v.x);
+    if (e == 4 || e == 12) { // +-i
+        v = s > 0.f ? make_float2(-v.y, v.x) : make_float2(v.y, -v.x);
     } else if (e == 8) {
         v = make_float2(-v.x, -v.y);
+    } else if (e % 4 == 2) { // c, s = +-H:  v (c + i s) = H (sc v + ss i v)
+        const float2 iv = make_float2(-v.y, v.x);
+        const float2 a = c > 0.f ? v : make_float2(-v.x, -v.y);
+        const float2 b = s > 0.f ? iv : make_float2(-iv.x, -iv.y);
+        v = mul2(make_float2(H, H), add2(a, b));
     } else {
-        v = make_float2(fmaf(-s, v.y, c * v.x), fmaf(s, v.x, c * v.y));
+        v = cmul(v, make_float2(c, s));
     }
 }
 

@@ -113,10 +113,10 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
 
     // ---- which tile
     long long t = blockIdx.x;
-    const long long cg = t % p.n_cgroups;
+    const long long cg = t % p.n_cgroups + p.cg0;
     t /= p.n_cgroups;
     const long long m = t % p.n_m;
-    const long long o = t / p.n_m;
+    const long long o = t / p.n_m + p.o0;
     const long long c0 = cg * p.nl;
     const int nl_eff = (int)((p.NC - c0) < (long long)p.nl ? (p.NC - c0) : (long long)p.nl);
     const long long base = o * p.SO + m * p.SM + c0 * p.SCc;
@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
         if (threadIdx.x == 0) {
             double tsum = 0.0;
             for (int w = 0; w < (int)(blockDim.x >> 5); ++w) tsum += red[w];
-            p.loss_scratch[blockIdx.x] = tsum;
+            p.loss_scratch[p.tile0 + blockIdx.x] = tsum;
         }
         __syncthreads();
     }

@@ -141,6 +141,15 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         const long long lines = col_type ? (a == 0 ? d.st : p->desc.nx) : p->desc.ny * (N / d.L);
         d.fast = !p->force_generic && pow2_supported(d.L, col_type) && lines % pow2_lines(d.L, col_type) == 0;
         if (d.fast) d.twg = pow2_group_twiddles(d.L);
+        if (d.fast && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
+            const long long Nj = d.L * d.st;
+            d.twb2.resize((size_t)Nj);
+            for (long long r = 0; r < d.st; ++r)
+                for (long long sl = 0; sl < d.L; ++sl) {
+                    const float2 w = d.twb[(size_t)((r * d.pi[(size_t)sl]) % Nj)];
+                    d.twb2[(size_t)(a == 1 ? r * d.L + sl : sl * d.st + r)] = w;
+                }
+        }
     }
     // slot -> true frequency index:  k = sum_j pi_j(p_j) (L_0 .. L_{j-1})
     ax.kslot.resize((size_t)N);
@@ -165,48 +174,57 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
     return true;
 }
 
-static PassTmpl mk(int axis, int digit, int d1, int d2, int ld, int mid, int st, const char* nm, double bpp)
+static PassTmpl mk(int axis, int digit, int d1, int d2, int ld, int mid, int st, const char* nm, double rd,
+                   double wr, double side = 0.0)
 {
     PassTmpl t;
     t.axis = axis; t.digit = digit; t.fft1_dir = d1; t.fft2_dir = d2;
-    t.load_op = ld; t.mid_op = mid; t.store_op = st; t.name = nm; t.bytes_per_point = bpp;
+    t.load_op = ld; t.mid_op = mid; t.store_op = st; t.name = nm;
+    t.rd = rd; t.wr = wr; t.side = side;
+    t.bytes_per_point = rd + wr + side;
     return t;
 }
 
 // passes of  F^-1{ mid (x) F{.} }  minus the first forward x digit and the last inverse x digit
-static void sandwich_core(const dop_plan* p, int mid, std::vector<PassTmpl>* out)
+static void sandwich_core(const dop_plan* p, int mid, bool with_xfwd, std::vector<PassTmpl>* out)
 {
     const int a = (int)p->ax[0].dig.size(), b = (int)p->ax[1].dig.size();
-    for (int j = 1; j < a; ++j) out->push_back(mk(0, j, +1, 0, LD_C64, MID_NONE, ST_C64, "x-fwd", 16));
-    for (int j = 0; j + 1 < b; ++j) out->push_back(mk(1, j, +1, 0, LD_C64, MID_NONE, ST_C64, "y-fwd", 16));
+    if (with_xfwd)
+        for (int j = 1; j < a; ++j) out->push_back(mk(0, j, +1, 0, LD_C64, MID_NONE, ST_C64, "x-fwd", 8, 8));
+    for (int j = 0; j + 1 < b; ++j) out->push_back(mk(1, j, +1, 0, LD_C64, MID_NONE, ST_C64, "y-fwd", 8, 8));
     out->push_back(mk(1, b - 1, +1, -1, LD_C64, mid, ST_C64,
-                      mid == MID_H ? "y-fwd*H*y-inv" : mid == MID_HCONJ ? "y-fwd*conjH*y-inv" : "y-fwd*G*y-inv", 16));
-    for (int j = b - 2; j >= 0; --j) out->push_back(mk(1, j, -1, 0, LD_C64, MID_NONE, ST_C64, "y-inv", 16));
-    for (int j = a - 1; j >= 1; --j) out->push_back(mk(0, j, -1, 0, LD_C64, MID_NONE, ST_C64, "x-inv", 16));
+                      mid == MID_H ? "y-fwd*H*y-inv" : mid == MID_HCONJ ? "y-fwd*conjH*y-inv" : "y-fwd*G*y-inv", 8, 8));
+    for (int j = b - 2; j >= 0; --j) out->push_back(mk(1, j, -1, 0, LD_C64, MID_NONE, ST_C64, "y-inv", 8, 8));
+    for (int j = a - 1; j >= 1; --j) out->push_back(mk(0, j, -1, 0, LD_C64, MID_NONE, ST_C64, "x-inv", 8, 8));
 }
 
 static void build_schedule(dop_plan* p)
 {
     const bool l2 = p->desc.loss == DOP_LOSS_L2;
     const bool wi = l2 && (p->desc.flags & DOP_WRITE_INTENSITY);
+    const int a = (int)p->ax[0].dig.size();
     p->fwd.clear(); p->adj.clear(); p->pre.clear();
     // forward
-    p->fwd.push_back(mk(0, 0, +1, 0, LD_HEIGHT, MID_NONE, ST_C64, "h->u0,x-fwd", 12));
-    sandwich_core(p, MID_H, &p->fwd);
+    p->fwd.push_back(mk(0, 0, +1, 0, LD_HEIGHT, MID_NONE, ST_C64, "h->u0,x-fwd", 4, 8));
+    sandwich_core(p, MID_H, true, &p->fwd);
     if (l2) {
-        p->fwd.push_back(mk(0, 0, -1, +1, LD_C64, MID_LOSS, ST_C64, "x-inv,|u|^2,loss,seed,x-fwd", wi ? 24 : 20));
+        // the seed's forward x transform belongs to the same row sandwich as the loss pass, so in
+        // L2 mode all of it runs inside dop_propagate_fwd (dop.h: the workspace then holds "the
+        // seeded, partly transformed gradient field")
+        p->fwd.push_back(mk(0, 0, -1, +1, LD_C64, MID_LOSS, ST_C64, "x-inv,|u|^2,loss,seed,x-fwd", 8, 8, wi ? 8 : 4));
+        for (int j = 1; j < a; ++j) p->fwd.push_back(mk(0, j, +1, 0, LD_C64, MID_NONE, ST_C64, "x-fwd", 8, 8));
     } else {
-        p->fwd.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_C64_INTENSITY, "x-inv,|u|^2", 20));
-        p->adj.push_back(mk(0, 0, +1, 0, LD_SEED, MID_NONE, ST_C64, "seed,x-fwd", 20));
+        p->fwd.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_C64_INTENSITY, "x-inv,|u|^2", 8, 8, 4));
+        p->adj.push_back(mk(0, 0, +1, 0, LD_SEED, MID_NONE, ST_C64, "seed,x-fwd", 8, 8, 4));
     }
     // adjoint
-    sandwich_core(p, MID_HCONJ, &p->adj);
-    p->adj.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_GRAD, "x-inv,grad", 16));
+    sandwich_core(p, MID_HCONJ, !l2, &p->adj);
+    p->adj.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_GRAD, "x-inv,grad", 8, 4, 4));
     // Gaussian pre-filter (real plane -> real plane through the complex field buffer)
     if (p->desc.prefilter_sigma_px > 0.0) {
-        p->pre.push_back(mk(0, 0, +1, 0, LD_REAL, MID_NONE, ST_C64, "real,x-fwd", 12));
-        sandwich_core(p, MID_GAUSS, &p->pre);
-        p->pre.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_REAL, "x-inv,real", 12));
+        p->pre.push_back(mk(0, 0, +1, 0, LD_REAL, MID_NONE, ST_C64, "real,x-fwd", 4, 8));
+        sandwich_core(p, MID_GAUSS, true, &p->pre);
+        p->pre.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_REAL, "x-inv,real", 8, 4));
     }
 }
 
@@ -260,6 +278,13 @@ dop_status build_plan(dop_plan* p)
     if (const char* e = std::getenv("DOP_TILE_PTS")) {
         int v = std::atoi(e);
         if (v >= 256 && v <= 16384) p->tile_pts = v;
+    }
+    // Multi-pass segments can run slab by slab so that the passes after the first hit L2.  Off by
+    // default: measured slower than whole-array launches on B200.
+    p->slab_bytes = 0;
+    if (const char* e = std::getenv("DOP_SLAB_MB")) {
+        int v = std::atoi(e);
+        if (v >= 0 && v <= 4096) p->slab_bytes = (long long)v << 20;
     }
     // generic kernel limits: a row-type line <= 8192 points (64 KiB), a column-type digit
     // <= 512 points (x 16 adjacent lines = 64 KiB)

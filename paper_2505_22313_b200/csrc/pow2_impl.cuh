@@ -1,0 +1,311 @@
+// pow2_impl.cuh -- register-blocked tile-pass kernels for power-of-two digits (the fast path).
+//
+// Same pass semantics and slot order as kernels_generic.cu (one CTA = one tile, one read + one
+// write of the field, fused pointwise ops; Eq. 1-4, PAPER.md:200 row-column 2-D
+// FFT), so a plan may mix the two kernel families pass by pass.  Every thread keeps 16 points in
+// registers (fft_regs.cuh) and moves them straight between registers and global memory:
+//   column-type tile: 16 adjacent lines x L slots, lanes run over the 16 lines (128-byte segments);
+//   row-type tile   : LINES contiguous lines of L points, lanes run over consecutive points.
+// Everything structural is a template parameter (digit length, tile type, fused-op variant,
+// boundary-twiddle mode), so the emitted code has no per-element branches and its addresses are
+// base + compile-time multiples of one stride.
+#pragma once
+#include "dop_internal.h"
+#include "fft_regs.cuh"
+
+namespace dop {
+
+using fx::P;
+
+// fused-op variants (what is fused around the digit DFT(s) of a pass)
+enum Variant : int {
+    V_FWD = 0,     // c64 -> DFT -> c64
+    V_INV = 1,     // c64 -> IDFT -> c64
+    V_LOSS = 2,    // c64 -> IDFT -> |u|^2, loss, seed -> DFT -> c64          (F6, F7, A1)
+    V_H = 3,       // c64 -> DFT -> (x) H or conj H -> IDFT -> c64            (F4 / A3)
+    V_GAUSS = 4,   // c64 -> DFT -> (x) Gaussian -> IDFT -> c64               (F0 / A6)
+    V_HEIGHT = 5,  // h -> exp(i Phi) -> DFT -> c64                           (F1, F2)
+    V_LDOTHER = 6, // seed (2 dL/dI u) or real plane -> DFT -> c64            (runtime load_op)
+    V_GRAD = 7,    // c64 -> IDFT -> dL/dh (+=)                               (A5)
+    V_STOTHER = 8  // c64 -> IDFT -> (u, |u|^2) or real plane                 (runtime store_op)
+};
+// boundary twiddle T_j = W_{N_j}^{k_j r_j} of a non-last digit
+enum TwbMode : int {
+    TWB_NONE = 0,
+    TWB_TILE = 1, // r_j is constant over the tile (y digits): table [r][slot], tile's row contiguous
+    TWB_LANE = 2  // r_j = the lane's line index (x digits):   table [slot][r], lanes coalesced
+};
+
+__host__ __device__ constexpr int variant_dir1(int v)
+{
+    return (v == V_FWD || v == V_H || v == V_GAUSS || v == V_HEIGHT || v == V_LDOTHER) ? +1 : -1;
+}
+__host__ __device__ constexpr int variant_dir2(int v) { return v == V_LOSS ? +1 : (v == V_H || v == V_GAUSS) ? -1 : 0; }
+
+__host__ __device__ constexpr int row_lines(int L) { return L >= 4096 ? 1 : 4096 / L; }
+__host__ __device__ constexpr int tile_threads(int L, bool col) { return col ? L : row_lines(L) * (L / P); }
+// resident CTAs per SM the register allocation is asked to allow
+__host__ __device__ constexpr int min_blocks(int L, bool col)
+{
+    return tile_threads(L, col) >= 512 ? 2 : 768 / tile_threads(L, col);
+}
+
+// F4 / A3: v *= H (or conj H) / N; evanescent bins (a < 0) zeroed.  a and the phase z sqrt(a)
+// are fp64; sqrt = fp32 rsqrt seed + two fp64 Newton steps.
+__device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double fy2, double z, float scale, bool conj)
+{
+    const double a = c_minus_fx2 - fy2; // (1/lambda^2 - fx^2) - fy^2, the definition's own order
+    if (a >= 0.0) {
+        double s = 0.0;
+        if (a > 0.0) {
+            const double y = (double)rsqrtf((float)a);
+            const double hy = 0.5 * y;
+            s = a * y;
+            s = fma(fma(-s, s, a), hy, s);
+            s = fma(fma(-s, s, a), hy, s);
+        }
+        const double turns = z * s;
+        const float f = (float)(turns - rint(turns)); // fractional turn, |f| <= 0.5
+        float sn, cs;
+        sincospif(2.0f * f, &sn, &cs);
+        const float2 h = make_float2(cs * scale, (conj ? -sn : sn) * scale);
+        return fx::cmul(v, h);
+    }
+    return make_float2(0.0f, 0.0f);
+}
+
+// ---- the tile-pass kernel -------------------------------------------------------------------
+template <int L, bool COL, int V, int TWB>
+__global__ void __launch_bounds__(tile_threads(L, COL), min_blocks(L, COL))
+pow2_kernel(const __grid_constant__ PassDesc p)
+{
+    using TL = fx::Tile<L, COL>;
+    using S = fx::Sched<L>;
+    constexpr int T = L / P;            // threads per line
+    constexpr int GL = S::NG - 1;       // last group
+    constexpr int RL = S::radix(GL);    // its radix
+    constexpr int DIR1 = variant_dir1(V), DIR2 = variant_dir2(V);
+    constexpr int LAST = DIR2 != 0 ? DIR2 : DIR1;
+    constexpr int LINES = row_lines(L);
+    extern __shared__ float2 s[];
+
+    // ---- which tile (same enumeration as the generic kernel)
+    long long t = blockIdx.x;
+    const long long cg = t % p.n_cgroups + p.cg0;
+    t /= p.n_cgroups;
+    const long long m = t % p.n_m;
+    const long long o = t / p.n_m + p.o0;
+    const int tid = threadIdx.x;
+    const int sub = COL ? (tid & 15) : (tid / T); // column in the bundle / line in the tile
+    const int tt = COL ? (tid >> 4) : (tid % T);
+    const long long line = cg * (COL ? 16 : LINES) + sub;
+    const long long es = COL ? p.es : 1;
+    const long long tbase = o * p.SO + m * p.SM + line * p.SCc;
+    const int soff = COL ? sub : sub * TL::LINE_ELEMS;
+    const float2* __restrict__ tw = p.tw_g;
+
+    // Register i holds slot tt + i T in the first group's layout and slot tt RL + kL(i) in the
+    // last group's (fft_regs.cuh Tile::slot with m = T resp. m = 1).
+    const long long b0 = tbase + (long long)tt * es;
+    const long long bL = tbase + (long long)(tt * RL) * es;
+#define DOP_K0(i) ((i) * T)
+#define DOP_KL(i) (((i) / RL) * (T * RL) + (i) % RL)
+
+    // boundary twiddle of the element in register i (last-group layout)
+    const float2* __restrict__ twp = nullptr;
+    unsigned tws = 1;
+    if (TWB == TWB_TILE) {
+        twp = p.tw_b2 + m * L + tt * RL;
+    } else if (TWB == TWB_LANE) {
+        tws = (unsigned)p.NC;
+        twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
+    }
+
+    float2 v[P];
+    // ---- load (+ prologue op, + conj boundary twiddle before an inverse DFT)
+    if (DIR1 > 0) {
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            const long long off = b0 + (long long)DOP_K0(i) * es;
+            if (V == V_HEIGHT) {
+                const float ph = __ldg(p.height + off) * p.phase_coef; // Eq. (1) in turns
+                sincospif(2.0f * ph, &v[i].y, &v[i].x);                // Eq. (2), E_in = 1
+            } else if (V == V_LDOTHER) {
+                if (p.load_op == LD_SEED) {
+                    const float2 u = p.field[off];
+                    const float g = 2.0f * __ldg(p.plane_in + off);
+                    v[i] = make_float2(g * u.x, g * u.y);
+                } else {
+                    v[i] = make_float2(__ldg(p.plane_in + off), 0.0f);
+                }
+            } else {
+                v[i] = p.field[off];
+            }
+        }
+    } else {
+        if (!COL && RL >= 2) {
+#pragma unroll
+            for (int i = 0; i < P; i += 2) {
+                const float4 q = *reinterpret_cast<const float4*>(p.field + bL + DOP_KL(i));
+                v[i] = make_float2(q.x, q.y);
+                v[i + 1] = make_float2(q.z, q.w);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < P; ++i) v[i] = p.field[bL + (long long)DOP_KL(i) * es];
+        }
+        if (TWB != TWB_NONE) {
+#pragma unroll
+            for (int i = 0; i < P; ++i) v[i] = fx::cmulc(v[i], __ldg(twp + (unsigned)DOP_KL(i) * tws));
+        }
+    }
+
+    if (DIR1 > 0) TL::template forward<0>(v, s, tt, soff, tw);
+    else TL::template inverse<GL>(v, s, tt, soff, tw);
+
+    // ---- middle op
+    if (V == V_H) { // registers hold spectrum slots in the last group's layout; this is the last y digit
+        const double* __restrict__ fyp = p.fy2 + o * p.row_o + m * p.row_m + tt * RL;
+        const double cfx = p.inv_lam2 - __ldg(p.fx2 + line);
+        const bool cj = p.mid_op == MID_HCONJ;
+#pragma unroll
+        for (int i = 0; i < P; ++i) v[i] = apply_h(v[i], cfx, __ldg(fyp + DOP_KL(i)), p.z, p.scale, cj);
+    } else if (V == V_GAUSS) {
+        const float* __restrict__ gyp = p.gy + o * p.row_o + m * p.row_m + tt * RL;
+        const float gxs = __ldg(p.gx + line) * p.scale;
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            const float g = gxs * __ldg(gyp + DOP_KL(i));
+            v[i] = make_float2(v[i].x * g, v[i].y * g);
+        }
+    } else if (V == V_LOSS) { // registers hold spatial points in the first group's layout
+        __shared__ double red[32];
+        double acc = 0.0;
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            const long long off = b0 + (long long)DOP_K0(i) * es;
+            const float I = v[i].x * v[i].x + v[i].y * v[i].y; // F6
+            const float d = I - __ldg(p.plane_in + off);       // F7
+            acc += (double)d * (double)d;
+            const float g = p.seed_coef * d;                    // A1: 2 gI = 4 (I - T)/N
+            v[i] = make_float2(g * v[i].x, g * v[i].y);
+            if (p.write_intensity) p.plane_out[off] = I;
+        }
+        // deterministic CTA reduction: warp shuffle tree, then thread 0 in warp order
+        for (int d = 16; d > 0; d >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, d);
+        if ((tid & 31) == 0) red[tid >> 5] = acc;
+        __syncthreads();
+        if (tid == 0) {
+            double r = 0.0;
+            constexpr int NW = (tile_threads(L, COL) + 31) / 32;
+            for (int w = 0; w < NW; ++w) r += red[w];
+            p.loss_scratch[p.tile0 + blockIdx.x] = r;
+        }
+    }
+
+    if (DIR2 > 0) TL::template forward<0>(v, s, tt, soff, tw);
+    else if (DIR2 < 0) TL::template inverse<GL>(v, s, tt, soff, tw);
+
+    // ---- store (+ boundary twiddle after a forward DFT, + epilogue op)
+    if (LAST > 0) {
+        if (TWB != TWB_NONE) {
+#pragma unroll
+            for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], __ldg(twp + (unsigned)DOP_KL(i) * tws));
+        }
+        if (!COL && RL >= 2) {
+#pragma unroll
+            for (int i = 0; i < P; i += 2)
+                *reinterpret_cast<float4*>(p.field + bL + DOP_KL(i)) = make_float4(v[i].x, v[i].y, v[i + 1].x, v[i + 1].y);
+        } else {
+#pragma unroll
+            for (int i = 0; i < P; ++i) p.field[bL + (long long)DOP_KL(i) * es] = v[i];
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            const long long off = b0 + (long long)DOP_K0(i) * es;
+            if (V == V_GRAD) {
+                const float ph = __ldg(p.height + off) * p.phase_coef;
+                float sn, cs;
+                sincospif(2.0f * ph, &sn, &cs); // u0 recomputed, not stored
+                float g = p.grad_coef * (cs * v[i].y - sn * v[i].x); // A5: c Im(conj(u0) g)
+                if (p.store_op == ST_GRAD_ACC) g += p.plane_out[off];
+                p.plane_out[off] = g;
+            } else if (V == V_STOTHER) {
+                if (p.store_op == ST_C64_INTENSITY) {
+                    p.field[off] = v[i];
+                    p.plane_out[off] = v[i].x * v[i].x + v[i].y * v[i].y;
+                } else {
+                    p.plane_out[off] = v[i].x;
+                }
+            } else {
+                p.field[off] = v[i];
+            }
+        }
+    }
+#undef DOP_K0
+#undef DOP_KL
+}
+
+// ---- host side -------------------------------------------------------------------------------
+template <int L, bool COL, int V, int TWB>
+static cudaError_t launch_one(const PassDesc& p, cudaStream_t stream)
+{
+    using TL = fx::Tile<L, COL>;
+    constexpr int threads = tile_threads(L, COL);
+    constexpr int smem = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
+    static bool attr_done = false; // per instantiation; the attribute is per device function
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 cudaSharedmemCarveoutMaxShared);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
+    if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
+    pow2_kernel<L, COL, V, TWB><<<(unsigned)ntiles, threads, smem, stream>>>(p);
+    return cudaGetLastError();
+}
+
+// All variants of one (L, tile type).  Returns cudaErrorInvalidValue for a combination that is
+// never scheduled (the dispatcher then falls back to the generic kernel).
+template <int L, bool COL>
+cudaError_t launch_L(const PassDesc& p, int variant, int twb, cudaStream_t st)
+{
+    if constexpr (COL) {
+        if (twb == TWB_NONE) {
+            if (variant == V_H) return launch_one<L, true, V_H, TWB_NONE>(p, st);
+            if (variant == V_GAUSS) return launch_one<L, true, V_GAUSS, TWB_NONE>(p, st);
+        } else if (twb == TWB_TILE) {
+            if (variant == V_FWD) return launch_one<L, true, V_FWD, TWB_TILE>(p, st);
+            if (variant == V_INV) return launch_one<L, true, V_INV, TWB_TILE>(p, st);
+        } else {
+            switch (variant) {
+            case V_FWD: return launch_one<L, true, V_FWD, TWB_LANE>(p, st);
+            case V_INV: return launch_one<L, true, V_INV, TWB_LANE>(p, st);
+            case V_LOSS: return launch_one<L, true, V_LOSS, TWB_LANE>(p, st);
+            case V_HEIGHT: return launch_one<L, true, V_HEIGHT, TWB_LANE>(p, st);
+            case V_LDOTHER: return launch_one<L, true, V_LDOTHER, TWB_LANE>(p, st);
+            case V_GRAD: return launch_one<L, true, V_GRAD, TWB_LANE>(p, st);
+            case V_STOTHER: return launch_one<L, true, V_STOTHER, TWB_LANE>(p, st);
+            }
+        }
+    } else {
+        if (twb == TWB_NONE) {
+            switch (variant) {
+            case V_FWD: return launch_one<L, false, V_FWD, TWB_NONE>(p, st);
+            case V_INV: return launch_one<L, false, V_INV, TWB_NONE>(p, st);
+            case V_LOSS: return launch_one<L, false, V_LOSS, TWB_NONE>(p, st);
+            case V_HEIGHT: return launch_one<L, false, V_HEIGHT, TWB_NONE>(p, st);
+            case V_LDOTHER: return launch_one<L, false, V_LDOTHER, TWB_NONE>(p, st);
+            case V_GRAD: return launch_one<L, false, V_GRAD, TWB_NONE>(p, st);
+            case V_STOTHER: return launch_one<L, false, V_STOTHER, TWB_NONE>(p, st);
+            }
+        }
+    }
+    return cudaErrorInvalidValue;
+}
+
+} // namespace dop
