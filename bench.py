@@ -137,6 +137,22 @@ def ncu_traffic(cfg_name: str, pass_name: str):
         return None
 
 
+def max_over_ranks(ms: float, dist, device) -> float:
+    """Multi-rank timing rule: every rank times its own replica on its device; the step time is the
+    MAX over ranks (all_reduce on `device`: a cuda device under nccl, 'cpu' under gloo in tests)."""
+    if dist is None:
+        return ms
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(points_per_replica: int, world: int, ms_per_step: float) -> float:
+    """Whole-job Gpoints/s of `world` independent replicas (weak scaling, no data-path collective)."""
+    return world * points_per_replica / (ms_per_step * 1e-3) / 1e9
+
+
 # ------------------------------------------------------------------------------------------------
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
@@ -241,12 +257,9 @@ def main():
     barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, dev)
     ms_per_step = ms / steps
-    value = world * points / (ms_per_step * 1e-3) / 1e9
+    value = aggregate_value(points, world, ms_per_step)
     loss_value = float(loss.item())
 
     # ---- per-launch CUDA events (same stream, same steps): the roofline of the dominant kernel
@@ -321,13 +334,10 @@ def main():
         e1.record(stream)
         barrier()
         ms2 = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms2], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms2 = float(t.item())
+        ms2 = max_over_ranks(ms2, dist, dev)
         h2d = h_host.numel() * 4 + T_host.numel() * 4
         d2h = g_host.numel() * 4 + 8 + (i_host.numel() * 4 if i_host is not None else 0)
-        e2e = {"value": world * points / (ms2 / e2e_steps * 1e-3) / 1e9, "unit": UNIT,
+        e2e = {"value": aggregate_value(points, world, ms2 / e2e_steps), "unit": UNIT,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
                "ms_per_step": ms2 / e2e_steps}
         del h_host, T_host, g_host, i_host

@@ -49,7 +49,7 @@ def _dep_stamp() -> str:
     for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS + ["pow2_inst.cu"]] + [os.path.abspath(__file__)]:
         with open(d, "rb") as f:
             h.update(f.read())
-    h.update(" ".join(NVCC_FLAGS).encode())
+    h.update((" ".join(NVCC_FLAGS) + os.environ.get("DOP_NVCC_EXTRA", "")).encode())
     return h.hexdigest()
 
 
@@ -68,6 +68,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJDIR, exist_ok=True)
     nvcc = _nvcc()
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("DOP_NVCC_EXTRA", "").split()  # tuning experiments, e.g. -DDOP_RESIDENT_THREADS=1024
 
     def compile_one(u):
         obj, src, flags = u

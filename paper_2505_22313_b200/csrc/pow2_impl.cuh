@@ -45,13 +45,41 @@ __host__ __device__ constexpr int variant_dir2(int v) { return v == V_LOSS ? +1 
 __host__ __device__ constexpr int row_lines(int L) { return L >= 4096 ? 1 : 4096 / L; }
 __host__ __device__ constexpr int tile_threads(int L, bool col) { return col ? L : row_lines(L) * (L / P); }
 // resident CTAs per SM the register allocation is asked to allow
+#ifndef DOP_RESIDENT_THREADS
+#define DOP_RESIDENT_THREADS 1024 // 65536 regs / 1024 threads -> 64 registers per thread (measured best: 768 -> 1024 gave C4 +10%)
+#endif
 __host__ __device__ constexpr int min_blocks(int L, bool col)
 {
-    return tile_threads(L, col) >= 512 ? 2 : 768 / tile_threads(L, col);
+    return tile_threads(L, col) >= 512 ? 2 : DOP_RESIDENT_THREADS / tile_threads(L, col);
+}
+
+// Cache-hinted global accesses as plain (non-volatile) asm so the unrolled loads can be scheduled
+// freely; the loaded field elements are overwritten later by this same thread (a data dependence).
+__device__ __forceinline__ float2 ld_cg(const float2* p) // L2 only: streaming field, keeps L1 for tables
+{
+    float2 v;
+    asm("ld.global.cg.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_cg(float2* p, float2 v)
+{
+    asm volatile("st.global.cg.v2.f32 [%0], {%1,%2};" ::"l"(p), "f"(v.x), "f"(v.y));
+}
+
+// Field accesses: column-type tiles stream through L2 only (each 128-byte segment is used once;
+// L1 is kept for the twiddle tables: y passes 0.244 -> 0.231 ms at C2).  Row-type tiles keep the
+// default policy; evict-first / L2-only hints on them and on the fp32 planes measured 10-40% slower.
+template <bool CG>
+__device__ __forceinline__ float2 field_ld(const float2* p) { return CG ? ld_cg(p) : *p; }
+template <bool CG>
+__device__ __forceinline__ void field_st(float2* p, float2 v)
+{
+    if (CG) st_cg(p, v);
+    else *p = v;
 }
 
 // F4 / A3: v *= H (or conj H) / N; evanescent bins (a < 0) zeroed.  a and the phase z sqrt(a)
-// are fp64; sqrt = fp32 rsqrt seed + two fp64 Newton steps.
+// are fp64; sqrt = fp32 rsqrt seed + one fp64 Newton step.
 __device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double fy2, double z, float scale, bool conj)
 {
     const double a = c_minus_fx2 - fy2; // (1/lambda^2 - fx^2) - fy^2, the definition's own order
@@ -60,9 +88,8 @@ __device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double f
         if (a > 0.0) {
             const double y = (double)rsqrtf((float)a);
             const double hy = 0.5 * y;
-            s = a * y;
-            s = fma(fma(-s, s, a), hy, s);
-            s = fma(fma(-s, s, a), hy, s);
+            s = a * y;                     // rel. error 2^-22 (fp32 rsqrt)
+            s = fma(fma(-s, s, a), hy, s); // one Newton step: ~3e-14, i.e. < 6e-9 turns at z sqrt(a) = 1.8e5
         }
         const double turns = z * s;
         const float f = (float)(turns - rint(turns)); // fractional turn, |f| <= 0.5
@@ -87,6 +114,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     constexpr int DIR1 = variant_dir1(V), DIR2 = variant_dir2(V);
     constexpr int LAST = DIR2 != 0 ? DIR2 : DIR1;
     constexpr int LINES = row_lines(L);
+    // L2-only field accesses: column tiles except the two variants where it measured slower (C4:
+    // loss pass 32 -> 45 ms, height pass 12.5 -> 13.7 ms)
+    constexpr bool CG = COL && V != V_LOSS && V != V_HEIGHT;
     extern __shared__ float2 s[];
 
     // ---- which tile (same enumeration as the generic kernel)
@@ -121,6 +151,17 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
 
+    // Touch the tables this tile will need after its DFT now, so they are in L1 by then.
+    if (TWB == TWB_TILE && LAST > 0) {
+#pragma unroll
+        for (int i = 0; i < P; i += (RL >= 16 ? 16 : RL)) asm volatile("prefetch.global.L1 [%0];" ::"l"(twp + DOP_KL(i)));
+    }
+    if (V == V_H) {
+        const double* fyp = p.fy2 + o * p.row_o + m * p.row_m + tt * RL;
+#pragma unroll
+        for (int i = 0; i < P; i += (RL >= 16 ? 16 : RL)) asm volatile("prefetch.global.L1 [%0];" ::"l"(fyp + DOP_KL(i)));
+    }
+
     float2 v[P];
     // ---- load (+ prologue op, + conj boundary twiddle before an inverse DFT)
     if (DIR1 > 0) {
@@ -132,27 +173,29 @@ pow2_kernel(const __grid_constant__ PassDesc p)
                 sincospif(2.0f * ph, &v[i].y, &v[i].x);                // Eq. (2), E_in = 1
             } else if (V == V_LDOTHER) {
                 if (p.load_op == LD_SEED) {
-                    const float2 u = p.field[off];
+                    const float2 u = field_ld<CG>(p.field + off);
                     const float g = 2.0f * __ldg(p.plane_in + off);
                     v[i] = make_float2(g * u.x, g * u.y);
                 } else {
                     v[i] = make_float2(__ldg(p.plane_in + off), 0.0f);
                 }
             } else {
-                v[i] = p.field[off];
+                v[i] = field_ld<CG>(p.field + off);
             }
         }
     } else {
         if (!COL && RL >= 2) {
 #pragma unroll
             for (int i = 0; i < P; i += 2) {
+                // default caching on purpose: a thread reads RL adjacent slots 16 bytes at a time, the
+                // rest of each 128-byte line is picked up from L1 by the following loads
                 const float4 q = *reinterpret_cast<const float4*>(p.field + bL + DOP_KL(i));
                 v[i] = make_float2(q.x, q.y);
                 v[i + 1] = make_float2(q.z, q.w);
             }
         } else {
 #pragma unroll
-            for (int i = 0; i < P; ++i) v[i] = p.field[bL + (long long)DOP_KL(i) * es];
+            for (int i = 0; i < P; ++i) v[i] = field_ld<CG>(p.field + bL + (long long)DOP_KL(i) * es);
         }
         if (TWB != TWB_NONE) {
 #pragma unroll
@@ -185,7 +228,7 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         for (int i = 0; i < P; ++i) {
             const long long off = b0 + (long long)DOP_K0(i) * es;
             const float I = v[i].x * v[i].x + v[i].y * v[i].y; // F6
-            const float d = I - __ldg(p.plane_in + off);       // F7
+            const float d = I - __ldg(p.plane_in + off);      // F7
             acc += (double)d * (double)d;
             const float g = p.seed_coef * d;                    // A1: 2 gI = 4 (I - T)/N
             v[i] = make_float2(g * v[i].x, g * v[i].y);
@@ -218,7 +261,7 @@ pow2_kernel(const __grid_constant__ PassDesc p)
                 *reinterpret_cast<float4*>(p.field + bL + DOP_KL(i)) = make_float4(v[i].x, v[i].y, v[i + 1].x, v[i + 1].y);
         } else {
 #pragma unroll
-            for (int i = 0; i < P; ++i) p.field[bL + (long long)DOP_KL(i) * es] = v[i];
+            for (int i = 0; i < P; ++i) field_st<CG>(p.field + bL + (long long)DOP_KL(i) * es, v[i]);
         }
     } else {
 #pragma unroll
@@ -229,17 +272,17 @@ pow2_kernel(const __grid_constant__ PassDesc p)
                 float sn, cs;
                 sincospif(2.0f * ph, &sn, &cs); // u0 recomputed, not stored
                 float g = p.grad_coef * (cs * v[i].y - sn * v[i].x); // A5: c Im(conj(u0) g)
-                if (p.store_op == ST_GRAD_ACC) g += p.plane_out[off];
+                if (p.store_op == ST_GRAD_ACC) g += __ldg(p.plane_out + off);
                 p.plane_out[off] = g;
             } else if (V == V_STOTHER) {
                 if (p.store_op == ST_C64_INTENSITY) {
-                    p.field[off] = v[i];
+                    field_st<CG>(p.field + off, v[i]);
                     p.plane_out[off] = v[i].x * v[i].x + v[i].y * v[i].y;
                 } else {
                     p.plane_out[off] = v[i].x;
                 }
             } else {
-                p.field[off] = v[i];
+                field_st<CG>(p.field + off, v[i]);
             }
         }
     }
