@@ -21,6 +21,7 @@ SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu"]
 # (column-type?, digit length) -- must match the DOP_DECL list in kernels_pow2.cu
 POW2_INST = [(1, L) for L in (16, 32, 64, 128, 256, 512)] + \
             [(0, L) for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192)]
+POW2_X3 = (16, 32, 64, 128)  # digits 3 * LP
 HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", os.path.join("..", "..", "include", "dop.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -38,6 +39,9 @@ def _nvcc() -> str:
 def _units():
     """(object path, source path, extra flags) of every translation unit."""
     units = [(os.path.join(OBJDIR, s.replace(".cu", ".o")), os.path.join(CSRC, s), []) for s in SOURCES]
+    for lp in POW2_X3:
+        units.append((os.path.join(OBJDIR, f"pow2_x3_{lp}.o"), os.path.join(CSRC, "pow2_inst.cu"),
+                      [f"-DDOP_INST_X3={lp}"]))
     for col, L in POW2_INST:
         units.append((os.path.join(OBJDIR, f"pow2_{'col' if col else 'row'}_{L}.o"),
                       os.path.join(CSRC, "pow2_inst.cu"), [f"-DDOP_INST_COL={col}", f"-DDOP_INST_L={L}"]))

@@ -10,9 +10,17 @@ DOP_DECL(16, true) DOP_DECL(32, true) DOP_DECL(64, true) DOP_DECL(128, true) DOP
 DOP_DECL(64, false) DOP_DECL(128, false) DOP_DECL(256, false) DOP_DECL(512, false) DOP_DECL(1024, false)
 DOP_DECL(2048, false) DOP_DECL(4096, false) DOP_DECL(8192, false)
 #undef DOP_DECL
+extern template cudaError_t launch_x3<16>(const PassDesc&, int, int, cudaStream_t);
+extern template cudaError_t launch_x3<32>(const PassDesc&, int, int, cudaStream_t);
+extern template cudaError_t launch_x3<64>(const PassDesc&, int, int, cudaStream_t);
+extern template cudaError_t launch_x3<128>(const PassDesc&, int, int, cudaStream_t);
 
 bool pow2_supported(long long L, bool col_type)
 {
+    if (col_type && L % 3 == 0) { // 3 * 2^k, k = 4..7: radix-3 step + three 2^k sub-tiles (plain passes only)
+        const long long lp = L / 3;
+        return lp >= 16 && lp <= 128 && (lp & (lp - 1)) == 0;
+    }
     if (L < 16 || (L & (L - 1)) != 0) return false;
     return col_type ? L <= 512 : (L >= 64 && L <= 8192);
 }
@@ -55,7 +63,14 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
         twb = p.r_from == 1 ? TWB_TILE : TWB_LANE;
     }
     cudaError_t e = cudaErrorInvalidValue;
-    if (col) {
+    if (p.L % 3 == 0) {
+        switch (p.L / 3) {
+        case 16: e = launch_x3<16>(p, v, twb, stream); break;
+        case 32: e = launch_x3<32>(p, v, twb, stream); break;
+        case 64: e = launch_x3<64>(p, v, twb, stream); break;
+        case 128: e = launch_x3<128>(p, v, twb, stream); break;
+        }
+    } else if (col) {
         switch (p.L) {
         case 16: e = launch_L<16, true>(p, v, twb, stream); break;
         case 32: e = launch_L<32, true>(p, v, twb, stream); break;
@@ -86,6 +101,7 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
 std::vector<float2> pow2_group_twiddles(long long L)
 {
     std::vector<float2> out;
+    if (L % 3 == 0) L /= 3; // digits 3 * 2^k: the tables of the 2^k sub-transform
     int lg = 0;
     while ((1LL << lg) < L) ++lg;
     const int n4 = lg / 2, n2 = lg & 1, nfull = n4 / 2, rlast = ((n4 & 1) ? 4 : 1) * (n2 ? 2 : 1);

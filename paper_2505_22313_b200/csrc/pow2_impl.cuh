@@ -290,6 +290,134 @@ pow2_kernel(const __grid_constant__ PassDesc p)
 #undef DOP_KL
 }
 
+// ---- digits of length 3 * 2^k: one radix-3 step fused in front of three register-blocked 2^k DFTs
+// Column-type tiles, plain forward / inverse passes only (the plan puts the factor 3 in a
+// non-last digit).  Slot order = the generic kernel's for the radix list (3, 4, 4, ...): slot
+// c LP + i' holds output k = c + 3 k'(i').  Each thread keeps the three sub-tiles (48 points).
+template <int LP, int V, int TWB>
+__global__ void __launch_bounds__(LP, (512 / LP) > 0 ? (512 / LP) : 1)
+pow2x3_kernel(const __grid_constant__ PassDesc p)
+{
+    using TL = fx::Tile<LP, true>;
+    using S = fx::Sched<LP>;
+    constexpr int T = LP / P;
+    constexpr int GL = S::NG - 1;
+    constexpr int RL = S::radix(GL);
+    constexpr int DIR = variant_dir1(V);
+    constexpr float HS3 = 0.86602540378443864676f; // sqrt(3)/2
+    extern __shared__ float2 s[];
+
+    long long t = blockIdx.x;
+    const long long cg = t % p.n_cgroups + p.cg0;
+    t /= p.n_cgroups;
+    const long long m = t % p.n_m;
+    const long long o = t / p.n_m + p.o0;
+    const int tid = threadIdx.x;
+    const int sub = tid & 15, tt = tid >> 4;
+    const long long line = cg * 16 + sub;
+    const long long es = p.es;
+    const long long tbase = o * p.SO + m * p.SM + line * p.SCc;
+    const float2* __restrict__ tw = p.tw_g;
+    const float2* __restrict__ wL = p.wL; // W_L^q, L = 3 LP
+#define DOP_K0(i) ((i) * T)
+#define DOP_KL(i) (((i) / RL) * (T * RL) + (i) % RL)
+    const float2* __restrict__ twp;
+    unsigned tws = 1;
+    if (TWB == TWB_TILE) {
+        twp = p.tw_b2 + m * (3 * LP) + tt * RL;
+    } else {
+        tws = (unsigned)p.NC;
+        twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
+    }
+
+    float2 v[3][P];
+    if (DIR > 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int i = 0; i < P; ++i) v[c][i] = ld_cg(p.field + tbase + (long long)(c * LP + tt + DOP_K0(i)) * es);
+        // radix-3 step (block length L, stride LP), outputs c = 1, 2 times W_L^{j c}
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            const int j = tt + DOP_K0(i);
+            const float2 a = v[0][i], b = v[1][i], c = v[2][i];
+            const float2 t1 = fx::cadd(b, c), d = fx::csub(b, c);
+            const float2 t2 = make_float2(a.x - 0.5f * t1.x, a.y - 0.5f * t1.y);
+            const float2 t3 = make_float2(HS3 * d.x, HS3 * d.y);
+            v[0][i] = fx::cadd(a, t1);
+            v[1][i] = fx::cmul(make_float2(t2.x + t3.y, t2.y - t3.x), __ldg(wL + j));     // t2 - i t3
+            v[2][i] = fx::cmul(make_float2(t2.x - t3.y, t2.y + t3.x), __ldg(wL + 2 * j)); // t2 + i t3
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            TL::template forward<0>(v[c], s, tt, sub, tw);
+#pragma unroll
+            for (int i = 0; i < P; ++i) {
+                const float2 w = __ldg(twp + (unsigned)(c * LP + DOP_KL(i)) * tws);
+                st_cg(p.field + tbase + (long long)(c * LP + tt * RL + DOP_KL(i)) * es, fx::cmul(v[c][i], w));
+            }
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+#pragma unroll
+            for (int i = 0; i < P; ++i) {
+                const float2 w = __ldg(twp + (unsigned)(c * LP + DOP_KL(i)) * tws);
+                v[c][i] = fx::cmulc(ld_cg(p.field + tbase + (long long)(c * LP + tt * RL + DOP_KL(i)) * es), w);
+            }
+            TL::template inverse<GL>(v[c], s, tt, sub, tw);
+        }
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            const int j = tt + DOP_K0(i);
+            const float2 a = v[0][i];
+            const float2 b = fx::cmulc(v[1][i], __ldg(wL + j));
+            const float2 c = fx::cmulc(v[2][i], __ldg(wL + 2 * j));
+            const float2 t1 = fx::cadd(b, c), d = fx::csub(b, c);
+            const float2 t2 = make_float2(a.x - 0.5f * t1.x, a.y - 0.5f * t1.y);
+            const float2 t3 = make_float2(HS3 * d.x, HS3 * d.y);
+            v[0][i] = fx::cadd(a, t1);
+            v[1][i] = make_float2(t2.x - t3.y, t2.y + t3.x); // inverse: t2 + i t3
+            v[2][i] = make_float2(t2.x + t3.y, t2.y - t3.x);
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int i = 0; i < P; ++i) st_cg(p.field + tbase + (long long)(c * LP + tt + DOP_K0(i)) * es, v[c][i]);
+    }
+#undef DOP_K0
+#undef DOP_KL
+}
+
+template <int LP, int V, int TWB>
+static cudaError_t launch_x3_one(const PassDesc& p, cudaStream_t stream)
+{
+    constexpr int smem = fx::Tile<LP, true>::LINE_ELEMS * (int)sizeof(float2);
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(pow2x3_kernel<LP, V, TWB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
+    if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
+    pow2x3_kernel<LP, V, TWB><<<(unsigned)ntiles, LP, smem, stream>>>(p);
+    return cudaGetLastError();
+}
+
+template <int LP>
+cudaError_t launch_x3(const PassDesc& p, int variant, int twb, cudaStream_t st)
+{
+    if (twb == TWB_TILE) {
+        if (variant == V_FWD) return launch_x3_one<LP, V_FWD, TWB_TILE>(p, st);
+        if (variant == V_INV) return launch_x3_one<LP, V_INV, TWB_TILE>(p, st);
+    } else if (twb == TWB_LANE) {
+        if (variant == V_FWD) return launch_x3_one<LP, V_FWD, TWB_LANE>(p, st);
+        if (variant == V_INV) return launch_x3_one<LP, V_INV, TWB_LANE>(p, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
 // ---- host side -------------------------------------------------------------------------------
 template <int L, bool COL, int V, int TWB>
 static cudaError_t launch_one(const PassDesc& p, cudaStream_t stream)
