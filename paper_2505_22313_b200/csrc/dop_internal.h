@@ -61,6 +61,7 @@ struct PassDesc {
     // ---- slab launch (a launch may cover only a range of column groups / outer indices)
     long long cg0, o0; // added to the decoded cg / o
     long long tile0;   // global tile index of this launch's first tile (loss partial slot)
+    int pf_ahead;      // pow2 kernels: CTA b prefetches the lines of tile b + pf_ahead into L2 (0 = off)
     // ---- in-tile DFT
     int n_radix;
     int radix[kMaxRadixSteps];
@@ -152,6 +153,7 @@ struct dop_plan {
     std::vector<long long> wl_len;
     std::vector<size_t> wl_off;
     int tile_pts = 4096;
+    int pf_waves = 1;           // L2 prefetch distance of the pow2 kernels, in waves of resident CTAs (0 = off)
     long long slab_bytes = 0;   // L2 slab size for multi-pass segments (0 = whole-array launches)
     bool force_generic = false; // DOP_FORCE_GENERIC at plan creation: generic kernel for every pass
     // schedules for one lambda

@@ -279,6 +279,10 @@ dop_status build_plan(dop_plan* p)
         int v = std::atoi(e);
         if (v >= 256 && v <= 16384) p->tile_pts = v;
     }
+    if (const char* e = std::getenv("DOP_PREFETCH_WAVES")) {
+        int v = std::atoi(e);
+        if (v >= 0 && v <= 64) p->pf_waves = v;
+    }
     // Multi-pass segments can run slab by slab so that the passes after the first hit L2.  Off by
     // default: measured slower than whole-array launches on B200.
     p->slab_bytes = 0;

@@ -66,6 +66,40 @@ __device__ __forceinline__ void st_cg(float2* p, float2 v)
     asm volatile("st.global.cg.v2.f32 [%0], {%1,%2};" ::"l"(p), "f"(v.x), "f"(v.y));
 }
 
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// Inter-CTA software pipelining: CTA b asks L2 for the lines that CTA b + pf_ahead (a couple of
+// waves later) will load, so DRAM keeps streaming while the resident CTAs compute and the later
+// CTA's loads are L2 hits.  One 128-byte line per thread covers the whole tile.
+template <bool COL, int THREADS, int NLINES, bool WANT_FIELD, bool WANT_HEIGHT, bool WANT_PLANE>
+__device__ __forceinline__ void prefetch_tile(const PassDesc& p, int slots_per_thread, int L)
+{
+    if (p.pf_ahead <= 0) return;
+    long long t = (long long)blockIdx.x + p.pf_ahead;
+    if (t >= (long long)gridDim.x) return;
+    const long long cg = t % p.n_cgroups + p.cg0;
+    t /= p.n_cgroups;
+    const long long m = t % p.n_m;
+    const long long o = t / p.n_m + p.o0;
+    const long long base = o * p.SO + m * p.SM + cg * NLINES * p.SCc;
+    const int tid = threadIdx.x;
+    if (COL) { // slot tid (+ k THREADS): 16 adjacent columns = one 128-byte line of the field
+        for (int k = 0; k < slots_per_thread; ++k) {
+            const long long off = base + (long long)(tid + k * THREADS) * p.es;
+            if (WANT_FIELD) prefetch_l2(p.field + off);
+            if (WANT_HEIGHT) prefetch_l2(p.height + off);
+            if (WANT_PLANE) prefetch_l2(p.plane_in + off);
+        }
+    } else { // the tile is NLINES * L contiguous points = THREADS lines of 16 complex64
+        const long long off = base + (long long)tid * 16;
+        if (WANT_FIELD) prefetch_l2(p.field + off);
+        if (tid * 32 < NLINES * L) {
+            if (WANT_HEIGHT) prefetch_l2(p.height + base + (long long)tid * 32);
+            if (WANT_PLANE) prefetch_l2(p.plane_in + base + (long long)tid * 32);
+        }
+    }
+}
+
 // Field accesses: column-type tiles stream through L2 only (each 128-byte segment is used once;
 // L1 is kept for the twiddle tables: y passes 0.244 -> 0.231 ms at C2).  Row-type tiles keep the
 // default policy; evict-first / L2-only hints on them and on the fp32 planes measured 10-40% slower.
@@ -76,6 +110,44 @@ __device__ __forceinline__ void field_st(float2* p, float2 v)
 {
     if (CG) st_cg(p, v);
     else *p = v;
+}
+
+// (cos 2 pi f, sin 2 pi f) for |f| <= 1/2 turn: quadrant q = round(4f) by the magic-number trick
+// (no F2I / FRND), residue |r| <= 1/8 turn, Taylor polynomials in r^2 (truncation 2e-9 / 2.4e-8),
+// then the quadrant rotation by selects and sign flips.  ~23 instructions against ~30 for the
+// library sincospif, which also has to handle arbitrary arguments.
+__device__ __forceinline__ void sincos_turn(float f, float* sn, float* cs)
+{
+#ifdef DOP_LIB_SINCOS
+    sincospif(2.0f * f, sn, cs);
+    return;
+#endif
+    const float MAGIC = 12582912.0f;                 // 1.5 * 2^23
+    const float t = fmaf(f, 4.0f, MAGIC);            // low mantissa bits = round(4 f) (two's complement)
+    const int q = __float_as_int(t);
+    const float r = fmaf(t - MAGIC, -0.25f, f);      // exact: f - q/4
+    const float r2 = r * r;
+    float sp = fmaf(r2, 42.05869394489765f, -76.70585975306136f);   // (2pi)^9/9!, -(2pi)^7/7!
+    sp = fmaf(sp, r2, 81.60524927607504f);                          // (2pi)^5/5!
+    sp = fmaf(sp, r2, -41.34170224039976f);                         // -(2pi)^3/3!
+    sp = fmaf(sp, r2, 6.283185307179586f);                          // 2pi
+    const float s = sp * r;
+    float cp = fmaf(r2, 60.24464137187666f, -85.45681720669373f);   // (2pi)^8/8!, -(2pi)^6/6!
+    cp = fmaf(cp, r2, 64.93939402266829f);                          // (2pi)^4/4!
+    cp = fmaf(cp, r2, -19.739208802178716f);                        // -(2pi)^2/2!
+    const float c = fmaf(cp, r2, 1.0f);
+    // q mod 4: 0 -> (c, s), 1 -> (-s, c), 2 -> (-c, -s), 3 -> (s, -c)
+    const bool odd = (q & 1) != 0;
+    const float co = odd ? s : c, so = odd ? c : s;
+    *cs = __int_as_float(__float_as_int(co) ^ (((q + 1) & 2) << 30));
+    *sn = __int_as_float(__float_as_int(so) ^ ((q & 2) << 30));
+}
+// the same for any moderate argument in turns (|ph| < 2^21): reduce to the nearest integer first
+__device__ __forceinline__ void sincos_turns(float ph, float* sn, float* cs)
+{
+    const float MAGIC = 12582912.0f;
+    const float n = (ph + MAGIC) - MAGIC; // round to nearest integer
+    sincos_turn(ph - n, sn, cs);
 }
 
 // F4 / A3: v *= H (or conj H) / N; evanescent bins (a < 0) zeroed.  a and the phase z sqrt(a)
@@ -92,9 +164,10 @@ __device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double f
             s = fma(fma(-s, s, a), hy, s); // one Newton step: ~3e-14, i.e. < 6e-9 turns at z sqrt(a) = 1.8e5
         }
         const double turns = z * s;
-        const float f = (float)(turns - rint(turns)); // fractional turn, |f| <= 0.5
+        const double RND = 6755399441055744.0;                    // 1.5 * 2^52: (x + RND) - RND = rint(x)
+        const float f = (float)(turns - ((turns + RND) - RND));   // fractional turn, |f| <= 0.5
         float sn, cs;
-        sincospif(2.0f * f, &sn, &cs);
+        sincos_turn(f, &sn, &cs);
         const float2 h = make_float2(cs * scale, (conj ? -sn : sn) * scale);
         return fx::cmul(v, h);
     }
@@ -151,6 +224,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
 
+    prefetch_tile<COL, tile_threads(L, COL), COL ? 16 : LINES, (V != V_HEIGHT && V != V_LDOTHER),
+                  (V == V_HEIGHT || V == V_GRAD), (V == V_LOSS)>(p, 1, L);
+
     // Touch the tables this tile will need after its DFT now, so they are in L1 by then.
     if (TWB == TWB_TILE && LAST > 0) {
 #pragma unroll
@@ -170,7 +246,7 @@ pow2_kernel(const __grid_constant__ PassDesc p)
             const long long off = b0 + (long long)DOP_K0(i) * es;
             if (V == V_HEIGHT) {
                 const float ph = __ldg(p.height + off) * p.phase_coef; // Eq. (1) in turns
-                sincospif(2.0f * ph, &v[i].y, &v[i].x);                // Eq. (2), E_in = 1
+                sincos_turns(ph, &v[i].y, &v[i].x);                // Eq. (2), E_in = 1
             } else if (V == V_LDOTHER) {
                 if (p.load_op == LD_SEED) {
                     const float2 u = field_ld<CG>(p.field + off);
@@ -270,7 +346,7 @@ pow2_kernel(const __grid_constant__ PassDesc p)
             if (V == V_GRAD) {
                 const float ph = __ldg(p.height + off) * p.phase_coef;
                 float sn, cs;
-                sincospif(2.0f * ph, &sn, &cs); // u0 recomputed, not stored
+                sincos_turns(ph, &sn, &cs); // u0 recomputed, not stored
                 float g = p.grad_coef * (cs * v[i].y - sn * v[i].x); // A5: c Im(conj(u0) g)
                 if (p.store_op == ST_GRAD_ACC) g += __ldg(p.plane_out + off);
                 p.plane_out[off] = g;
@@ -329,6 +405,8 @@ pow2x3_kernel(const __grid_constant__ PassDesc p)
         tws = (unsigned)p.NC;
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
+
+    prefetch_tile<true, LP, 16, true, false, false>(p, 3, 3 * LP);
 
     float2 v[3][P];
     if (DIR > 0) {
