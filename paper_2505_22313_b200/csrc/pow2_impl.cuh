@@ -48,9 +48,16 @@ __host__ __device__ constexpr int tile_threads(int L, bool col) { return col ? L
 #ifndef DOP_RESIDENT_THREADS
 #define DOP_RESIDENT_THREADS 1024 // 65536 regs / 1024 threads -> 64 registers per thread (measured best: 768 -> 1024 gave C4 +10%)
 #endif
-__host__ __device__ constexpr int min_blocks(int L, bool col)
+#ifndef DOP_LOSS_THREADS
+#define DOP_LOSS_THREADS DOP_RESIDENT_THREADS
+#endif
+#ifndef DOP_HEAVY_THREADS
+#define DOP_HEAVY_THREADS DOP_RESIDENT_THREADS // register budget of the loss / H / Gaussian variants
+#endif
+__host__ __device__ constexpr int min_blocks(int L, bool col, int v = 0)
 {
-    return tile_threads(L, col) >= 512 ? 2 : DOP_RESIDENT_THREADS / tile_threads(L, col);
+    const int rt = v == 2 ? DOP_LOSS_THREADS : (v == 3 || v == 4) ? DOP_HEAVY_THREADS : DOP_RESIDENT_THREADS;
+    return tile_threads(L, col) >= 512 ? 2 : (rt / tile_threads(L, col) > 0 ? rt / tile_threads(L, col) : 1);
 }
 
 // Cache-hinted global accesses as plain (non-volatile) asm so the unrolled loads can be scheduled
@@ -74,6 +81,9 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 template <bool COL, int THREADS, int NLINES, bool WANT_FIELD, bool WANT_HEIGHT, bool WANT_PLANE>
 __device__ __forceinline__ void prefetch_tile(const PassDesc& p, int slots_per_thread, int L)
 {
+#ifdef DOP_NO_PF
+    return;
+#endif
     if (p.pf_ahead <= 0) return;
     long long t = (long long)blockIdx.x + p.pf_ahead;
     if (t >= (long long)gridDim.x) return;
@@ -176,7 +186,7 @@ __device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double f
 
 // ---- the tile-pass kernel -------------------------------------------------------------------
 template <int L, bool COL, int V, int TWB>
-__global__ void __launch_bounds__(tile_threads(L, COL), min_blocks(L, COL))
+__global__ void __launch_bounds__(tile_threads(L, COL), min_blocks(L, COL, V))
 pow2_kernel(const __grid_constant__ PassDesc p)
 {
     using TL = fx::Tile<L, COL>;
@@ -224,8 +234,11 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
 
-    prefetch_tile<COL, tile_threads(L, COL), COL ? 16 : LINES, (V != V_HEIGHT && V != V_LDOTHER),
-                  (V == V_HEIGHT || V == V_GRAD), (V == V_LOSS)>(p, 1, L);
+    // (not compiled into the x column tiles: it never pays there and its registers cost the loss
+    // variant 25%, C4 32 -> 41 ms)
+    if (!COL || TWB != TWB_LANE)
+        prefetch_tile<COL, tile_threads(L, COL), COL ? 16 : LINES, (V != V_HEIGHT && V != V_LDOTHER),
+                      (V == V_HEIGHT || V == V_GRAD), (V == V_LOSS)>(p, 1, L);
 
     // Touch the tables this tile will need after its DFT now, so they are in L1 by then.
     if (TWB == TWB_TILE && LAST > 0) {
