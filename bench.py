@@ -129,12 +129,20 @@ def measured_peak_gbs():
 
 
 def ncu_traffic(cfg_name: str, pass_name: str):
-    """dram bytes per launch of the dominant pass from the committed ncu capture, if any."""
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant pass from
+    the committed `ncu --set full` capture (profiles/traffic.csv: config,pass,bytes), if any."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(cfg_name, {}).get(pass_name)
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f:
+                if line.startswith("#") or line.count(",") < 2:
+                    continue
+                cfg, rest = line.strip().split(",", 1)      # pass names contain commas:
+                name, nbytes = rest.rsplit(",", 1)           # config , pass ... , bytes
+                if cfg == cfg_name and name == pass_name:
+                    return float(nbytes)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def max_over_ranks(ms: float, dist, device) -> float:
