@@ -49,7 +49,7 @@ __host__ __device__ constexpr int tile_threads(int L, bool col) { return col ? L
 #define DOP_RESIDENT_THREADS 1024 // 65536 regs / 1024 threads -> 64 registers per thread (measured best: 768 -> 1024 gave C4 +10%)
 #endif
 #ifndef DOP_LOSS_THREADS
-#define DOP_LOSS_THREADS DOP_RESIDENT_THREADS
+#define DOP_LOSS_THREADS 512 // the loss variant keeps 16 points + 16 target values live: 128 registers, no spill
 #endif
 #ifndef DOP_HEAVY_THREADS
 #define DOP_HEAVY_THREADS DOP_RESIDENT_THREADS // register budget of the loss / H / Gaussian variants
@@ -203,11 +203,13 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     extern __shared__ float2 s[];
 
     // ---- which tile (same enumeration as the generic kernel)
-    long long t = blockIdx.x;
-    const long long cg = t % p.n_cgroups + p.cg0;
-    t /= p.n_cgroups;
-    const long long m = t % p.n_m;
-    const long long o = t / p.n_m + p.o0;
+    // (32-bit divisions: the launcher guarantees fewer than 2^31 tiles)
+    unsigned t = blockIdx.x;
+    const unsigned ncg = (unsigned)p.n_cgroups, nm = (unsigned)p.n_m;
+    const long long cg = (long long)(t % ncg) + p.cg0;
+    t /= ncg;
+    const long long m = t % nm;
+    const long long o = (long long)(t / nm) + p.o0;
     const int tid = threadIdx.x;
     const int sub = COL ? (tid & 15) : (tid / T); // column in the bundle / line in the tile
     const int tt = COL ? (tid >> 4) : (tid % T);
@@ -223,6 +225,11 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     const long long bL = tbase + (long long)(tt * RL) * es;
 #define DOP_K0(i) ((i) * T)
 #define DOP_KL(i) (((i) / RL) * (T * RL) + (i) % RL)
+    // Addresses are walked with running offsets (one 64-bit add per access) rather than
+    // i * stride products: the stride of a column tile is a run-time 64-bit value.
+    const long long step0 = (long long)T * es;                  // first-group layout: register i -> i + 1
+    const long long stepLr = (long long)(T * RL - (RL - 1)) * es; // last-group layout: end of a run of RL -> next run
+#define DOP_NEXT_L(ptr, i) ptr += ((((i) % RL) == RL - 1) ? stepLr : es)
 
     // boundary twiddle of the element in register i (last-group layout)
     const float2* __restrict__ twp = nullptr;
@@ -254,9 +261,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     float2 v[P];
     // ---- load (+ prologue op, + conj boundary twiddle before an inverse DFT)
     if (DIR1 > 0) {
+        long long off = b0;
 #pragma unroll
-        for (int i = 0; i < P; ++i) {
-            const long long off = b0 + (long long)DOP_K0(i) * es;
+        for (int i = 0; i < P; ++i, off += step0) {
             if (V == V_HEIGHT) {
                 const float ph = __ldg(p.height + off) * p.phase_coef; // Eq. (1) in turns
                 sincos_turns(ph, &v[i].y, &v[i].x);                // Eq. (2), E_in = 1
@@ -283,8 +290,12 @@ pow2_kernel(const __grid_constant__ PassDesc p)
                 v[i + 1] = make_float2(q.z, q.w);
             }
         } else {
+            const float2* lp = p.field + bL;
 #pragma unroll
-            for (int i = 0; i < P; ++i) v[i] = field_ld<CG>(p.field + bL + (long long)DOP_KL(i) * es);
+            for (int i = 0; i < P; ++i) {
+                v[i] = field_ld<CG>(lp);
+                DOP_NEXT_L(lp, i);
+            }
         }
         if (TWB != TWB_NONE) {
 #pragma unroll
@@ -313,9 +324,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     } else if (V == V_LOSS) { // registers hold spatial points in the first group's layout
         __shared__ double red[32];
         double acc = 0.0;
+        long long off = b0;
 #pragma unroll
-        for (int i = 0; i < P; ++i) {
-            const long long off = b0 + (long long)DOP_K0(i) * es;
+        for (int i = 0; i < P; ++i, off += step0) {
             const float I = v[i].x * v[i].x + v[i].y * v[i].y; // F6
             const float d = I - __ldg(p.plane_in + off);      // F7
             acc += (double)d * (double)d;
@@ -349,13 +360,17 @@ pow2_kernel(const __grid_constant__ PassDesc p)
             for (int i = 0; i < P; i += 2)
                 *reinterpret_cast<float4*>(p.field + bL + DOP_KL(i)) = make_float4(v[i].x, v[i].y, v[i + 1].x, v[i + 1].y);
         } else {
+            float2* sp = p.field + bL;
 #pragma unroll
-            for (int i = 0; i < P; ++i) field_st<CG>(p.field + bL + (long long)DOP_KL(i) * es, v[i]);
+            for (int i = 0; i < P; ++i) {
+                field_st<CG>(sp, v[i]);
+                DOP_NEXT_L(sp, i);
+            }
         }
     } else {
+        long long off = b0;
 #pragma unroll
-        for (int i = 0; i < P; ++i) {
-            const long long off = b0 + (long long)DOP_K0(i) * es;
+        for (int i = 0; i < P; ++i, off += step0) {
             if (V == V_GRAD) {
                 const float ph = __ldg(p.height + off) * p.phase_coef;
                 float sn, cs;
@@ -377,6 +392,7 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     }
 #undef DOP_K0
 #undef DOP_KL
+#undef DOP_NEXT_L
 }
 
 // ---- digits of length 3 * 2^k: one radix-3 step fused in front of three register-blocked 2^k DFTs
