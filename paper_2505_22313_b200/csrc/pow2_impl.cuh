@@ -85,12 +85,13 @@ __device__ __forceinline__ void prefetch_tile(const PassDesc& p, int slots_per_t
     return;
 #endif
     if (p.pf_ahead <= 0) return;
-    long long t = (long long)blockIdx.x + p.pf_ahead;
-    if (t >= (long long)gridDim.x) return;
-    const long long cg = t % p.n_cgroups + p.cg0;
-    t /= p.n_cgroups;
-    const long long m = t % p.n_m;
-    const long long o = t / p.n_m + p.o0;
+    unsigned t = blockIdx.x + (unsigned)p.pf_ahead;
+    if (t >= gridDim.x) return;
+    const unsigned ncg = (unsigned)p.n_cgroups, nm = (unsigned)p.n_m;
+    const long long cg = (long long)(t % ncg) + p.cg0;
+    t /= ncg;
+    const long long m = t % nm;
+    const long long o = (long long)(t / nm) + p.o0;
     const long long base = o * p.SO + m * p.SM + cg * NLINES * p.SCc;
     const int tid = threadIdx.x;
     if (COL) { // slot tid (+ k THREADS): 16 adjacent columns = one 128-byte line of the field
@@ -412,11 +413,12 @@ pow2x3_kernel(const __grid_constant__ PassDesc p)
     constexpr float HS3 = 0.86602540378443864676f; // sqrt(3)/2
     extern __shared__ float2 s[];
 
-    long long t = blockIdx.x;
-    const long long cg = t % p.n_cgroups + p.cg0;
-    t /= p.n_cgroups;
-    const long long m = t % p.n_m;
-    const long long o = t / p.n_m + p.o0;
+    unsigned t = blockIdx.x;
+    const unsigned ncg = (unsigned)p.n_cgroups, nm = (unsigned)p.n_m;
+    const long long cg = (long long)(t % ncg) + p.cg0;
+    t /= ncg;
+    const long long m = t % nm;
+    const long long o = (long long)(t / nm) + p.o0;
     const int tid = threadIdx.x;
     const int sub = tid & 15, tt = tid >> 4;
     const long long line = cg * 16 + sub;
