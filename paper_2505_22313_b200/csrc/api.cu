@@ -190,6 +190,31 @@ void prof_end(dop_plan* p, long long slot, cudaStream_t st)
 long long gcdll(long long a, long long b) { while (b) { long long t = a % b; a = b; b = t; } return a; }
 long long lcmll(long long a, long long b) { return a / gcdll(a, b) * b; }
 
+
+// Slab unit (columns for y segments, rows for x segments) and slab size of a segment; false when the
+// segment runs as whole-array launches.
+template <class D>
+bool slab_layout(const dop_plan* p, const std::vector<D>& d, int axis, long long* total, long long* per)
+{
+    const long long nx = p->desc.nx, ny = p->desc.ny;
+    *total = axis == 1 ? nx : ny;
+    *per = *total;
+    if (!(p->slab_bytes > 0 && d.size() >= 2)) return false;
+    long long unit = 1;
+    for (const D& q : d) {
+        if (axis == 1) unit = lcmll(unit, q.nl);
+        else if (!q.col_type) {
+            const long long lpr = nx / q.L; // lines per row
+            if (q.nl > lpr) unit = lcmll(unit, (q.nl + lpr - 1) / lpr);
+        }
+    }
+    const long long group_bytes = (axis == 1 ? ny : nx) * (long long)sizeof(float2);
+    *per = p->slab_bytes / group_bytes / unit * unit;
+    if (*per < unit) *per = unit;
+    if (*per >= *total) { *per = *total; return false; }
+    return true;
+}
+
 std::string pass_label(const char* tag, const PassTmpl& t)
 {
     return std::string(tag) + ":" + (t.axis == 0 ? "x" : "y") + std::to_string(t.digit) + ":" + t.name;
@@ -206,23 +231,9 @@ dop_status run_segment(dop_plan* p, const std::vector<PassTmpl>& sched, size_t b
     const int axis = sched[b].axis;
     std::vector<PassDesc> d;
     for (size_t i = b; i < e; ++i) d.push_back(resolve(p, sched[i], lam, bufs, ws));
-    // slab unit (columns for y segments, rows for x segments) and slab size
-    long long unit = 1, total = axis == 1 ? nx : ny, per = total;
-    const bool slabbed = p->slab_bytes > 0 && e - b >= 2;
-    if (slabbed) {
-        for (const PassDesc& q : d) {
-            if (axis == 1) unit = lcmll(unit, q.nl);
-            else if (!q.col_type) {
-                const long long lpr = nx / q.L; // lines per row
-                if (q.nl > lpr) unit = lcmll(unit, (q.nl + lpr - 1) / lpr);
-            }
-        }
-        const long long group_bytes = (axis == 1 ? ny : nx) * (long long)sizeof(float2);
-        per = p->slab_bytes / group_bytes / unit * unit;
-        if (per < unit) per = unit;
-        if (per > total) per = total;
-    }
-    if (!slabbed || per >= total) { // whole-array launches, one profiling slot per launch
+    long long total = 0, per = 0;
+    const bool slabbed = slab_layout(p, d, axis, &total, &per);
+    if (!slabbed) { // whole-array launches, one profiling slot per launch
         for (size_t i = b; i < e; ++i) {
             long long slot = prof_begin(p, pass_label(tag, sched[i]), sched[i].bytes_per_point, st);
             cudaError_t er = launch_tile_pass(d[i - b], st);
@@ -230,6 +241,18 @@ dop_status run_segment(dop_plan* p, const std::vector<PassTmpl>& sched, size_t b
             if (er != cudaSuccess) return DOP_ERR_CUDA;
         }
         return DOP_OK;
+    }
+    // lazily create the auxiliary streams (DOP_SLAB_STREAMS, default 2)
+    if (p->n_aux == 0) {
+        int ns = 2;
+        if (const char* e = std::getenv("DOP_SLAB_STREAMS")) ns = std::atoi(e);
+        ns = ns < 1 ? 1 : (ns > 4 ? 4 : ns);
+        if (cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess) return DOP_ERR_CUDA;
+        for (int k = 0; k < ns; ++k) {
+            if (cudaStreamCreateWithFlags(&p->aux[k], cudaStreamNonBlocking) != cudaSuccess) return DOP_ERR_CUDA;
+            if (cudaEventCreateWithFlags(&p->ev_join[k], cudaEventDisableTiming) != cudaSuccess) return DOP_ERR_CUDA;
+        }
+        p->n_aux = ns;
     }
     std::string name = std::string(tag) + ":" + (axis == 0 ? "x" : "y") + "-seg[";
     double dram = sched[b].rd + sched[e - 1].wr;
@@ -239,7 +262,12 @@ dop_status run_segment(dop_plan* p, const std::vector<PassTmpl>& sched, size_t b
     }
     name += "]";
     long long slot = prof_begin(p, name, dram, st);
-    for (long long g0 = 0; g0 < total; g0 += per) {
+    if (cudaEventRecord(p->ev_fork, st) != cudaSuccess) return DOP_ERR_CUDA;
+    for (int k = 0; k < p->n_aux; ++k)
+        if (cudaStreamWaitEvent(p->aux[k], p->ev_fork, 0) != cudaSuccess) return DOP_ERR_CUDA;
+    long long slab_index = 0;
+    for (long long g0 = 0; g0 < total; g0 += per, ++slab_index) {
+        cudaStream_t ss = p->aux[slab_index % p->n_aux];
         const long long g1 = g0 + per < total ? g0 + per : total;
         for (PassDesc q : d) {
             if (axis == 1) { // columns [g0, g1)
@@ -255,8 +283,12 @@ dop_status run_segment(dop_plan* p, const std::vector<PassTmpl>& sched, size_t b
                 q.n_cgroups = ((g1 - g0) * lpr + q.nl - 1) / q.nl;
                 q.tile0 = q.cg0;
             }
-            if (launch_tile_pass(q, st) != cudaSuccess) return DOP_ERR_CUDA;
+            if (launch_tile_pass(q, ss) != cudaSuccess) return DOP_ERR_CUDA;
         }
+    }
+    for (int k = 0; k < p->n_aux; ++k) {
+        if (cudaEventRecord(p->ev_join[k], p->aux[k]) != cudaSuccess) return DOP_ERR_CUDA;
+        if (cudaStreamWaitEvent(st, p->ev_join[k], 0) != cudaSuccess) return DOP_ERR_CUDA;
     }
     prof_end(p, slot, st);
     return DOP_OK;
@@ -386,6 +418,11 @@ dop_status dop_plan_destroy(dop_plan* p)
 {
     if (p == nullptr) return DOP_ERR_INVALID_ARG;
     if (p->d_arena != nullptr) cudaFree(p->d_arena);
+    for (int k = 0; k < p->n_aux; ++k) {
+        if (p->aux[k]) cudaStreamDestroy(p->aux[k]);
+        if (p->ev_join[k]) cudaEventDestroy(p->ev_join[k]);
+    }
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     for (cudaEvent_t e : p->ev_start) cudaEventDestroy(e);
     for (cudaEvent_t e : p->ev_stop) cudaEventDestroy(e);
     delete p;
@@ -421,7 +458,22 @@ size_t dop_plan_describe(const dop_plan* p, char* buf, size_t len)
 int64_t dop_plan_launch_count(const dop_plan* p)
 {
     if (p == nullptr) return 0;
-    int64_t n = (int64_t)(p->fwd.size() + p->adj.size()) * p->desc.n_lambda + 2 * (int64_t)p->pre.size();
+    auto count = [&](const std::vector<PassTmpl>& sched) {
+        int64_t n = 0;
+        size_t i = 0;
+        while (i < sched.size()) {
+            size_t j = i + 1;
+            while (j < sched.size() && sched[j].axis == sched[i].axis) ++j;
+            std::vector<PassDesc> d(j - i);
+            for (size_t k = i; k < j; ++k) tile_geometry(p, sched[k].axis, sched[k].digit, &d[k - i]);
+            long long total = 0, per = 0;
+            const bool slabbed = slab_layout(p, d, sched[i].axis, &total, &per);
+            n += (int64_t)(j - i) * (slabbed ? (total + per - 1) / per : 1);
+            i = j;
+        }
+        return n;
+    };
+    int64_t n = (count(p->fwd) + count(p->adj)) * p->desc.n_lambda + 2 * count(p->pre);
     if (p->desc.loss == DOP_LOSS_L2) n += 1;
     return n;
 }

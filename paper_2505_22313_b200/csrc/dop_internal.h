@@ -170,6 +170,11 @@ struct dop_plan {
     float* d_g[2] = {nullptr, nullptr};
     std::vector<size_t> pi_off[2];
     int state = 0; // 1 after a successful fwd
+    // slab schedule: auxiliary streams the slabs of a segment are dealt to, so that the launch tails of
+    // one slab overlap the next slab's kernels (fork / join around the segment on the caller's stream)
+    int n_aux = 0;
+    cudaStream_t aux[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[4] = {nullptr, nullptr, nullptr, nullptr};
     // per-launch profiling (dop_plan_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_start, ev_stop;

@@ -127,3 +127,20 @@ def test_no_cpu_fallback_without_a_device():
         assert st in (dop.DOP_ERR_CUDA, dop.DOP_ERR_ARCH)
     finally:
         dop.dop_plan_destroy(plan)
+
+
+def test_launch_count_follows_the_slab_schedule(monkeypatch):
+    """dop_plan_launch_count is exact for whole-array launches and for the slab schedule."""
+    args = (1024, 2048, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0)
+    monkeypatch.setenv("DOP_XDIGITS", "16,128")
+    monkeypatch.delenv("DOP_SLAB_MB", raising=False)
+    h, _ = dop.dop_plan_create(*args)
+    base = dop.dop_plan_launch_count(h)
+    dop.dop_plan_destroy(h)
+    assert base == 13 + 1  # 13 passes (x 16.128, y 32.32) + the loss reduction
+    monkeypatch.setenv("DOP_SLAB_MB", "1")
+    h, _ = dop.dop_plan_create(*args)
+    n = dop.dop_plan_launch_count(h)
+    dop.dop_plan_destroy(h)
+    # x segments: rows of 16 KiB -> 64 rows per slab -> 16 slabs; y segments: columns of 8 KiB -> 128 -> 16 slabs
+    assert n == 13 * 16 + 1

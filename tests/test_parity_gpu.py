@@ -127,6 +127,23 @@ def test_every_digit_decomposition_gives_the_same_answer(env, monkeypatch):
     assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
 
 
+def test_slab_schedule_gives_the_same_answer(monkeypatch):
+    """DOP_SLAB_MB: multi-pass segments run slab by slab on auxiliary streams (fork / join on the
+    caller's stream); 1 MiB slabs split this grid into 16 column slabs and 16 row slabs."""
+    monkeypatch.setenv("DOP_XDIGITS", "16,128")
+    cfg = synth.CONFIGS["C4"].scaled(1024, 2048)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I0, L0, g0 = run_l2(cfg, h, T)
+    monkeypatch.setenv("DOP_SLAB_MB", "1")
+    I1, L1, g1 = run_l2(cfg, h, T)
+    # same kernels on the same tiles, only the launch grouping differs: bit-identical
+    assert np.array_equal(I0, I1) and np.array_equal(g0, g1) and L0 == L1
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I1, Ir, "intensity")
+    check(g1, gr, "dL/dh")
+    assert abs(L1 - Lr) <= TOL_LOSS * abs(Lr)
+
+
 def test_degenerate_inputs():
     """z = 0 (identity on a grid without evanescent bins), flat height (plane wave), negative z."""
     cfg = synth.CONFIGS["C1"].scaled(64, 96)
