@@ -201,6 +201,12 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     // L2-only field accesses: column tiles except the two variants where it measured slower (C4:
     // loss pass 32 -> 45 ms, height pass 12.5 -> 13.7 ms)
     constexpr bool CG = COL && V != V_LOSS && V != V_HEIGHT;
+    // Row tiles whose last group is radix 16: a thread owns 16 adjacent slots (128 bytes) and a warp 4 KiB of
+    // contiguous memory.  Its global accesses are staged through a padded per-warp shared-memory
+    // buffer so that every LDG/STG.128 of the warp covers 512 contiguous bytes instead of 16 bytes
+    // in each of 32 lines.
+    constexpr bool STAGE = !COL && RL == 16;
+    constexpr int STG_LANE = 16 * 8 + 16; // bytes per lane: 128 + 16 padding (conflict-free both ways)
     extern __shared__ float2 s[];
 
     // ---- which tile (same enumeration as the generic kernel)
@@ -281,7 +287,24 @@ pow2_kernel(const __grid_constant__ PassDesc p)
             }
         }
     } else {
-        if (!COL && RL >= 2) {
+        if (STAGE) {
+            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * (32 * STG_LANE);
+            const int lane = tid & 31;
+            const char* g0 = reinterpret_cast<const char*>(p.field + bL - lane * 16); // the warp's 4 KiB
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float4 q = *reinterpret_cast<const float4*>(g0 + j * 512 + lane * 16);
+                *reinterpret_cast<float4*>(wb + (4 * j + (lane >> 3)) * STG_LANE + (lane & 7) * 16) = q;
+            }
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float4 q = *reinterpret_cast<const float4*>(wb + lane * STG_LANE + j * 16);
+                v[2 * j] = make_float2(q.x, q.y);
+                v[2 * j + 1] = make_float2(q.z, q.w);
+            }
+            __syncthreads(); // the staging area overlaps the exchange buffer of the DFT below
+        } else if (!COL && RL >= 2) {
 #pragma unroll
             for (int i = 0; i < P; i += 2) {
                 // default caching on purpose: a thread reads RL adjacent slots 16 bytes at a time, the
@@ -356,7 +379,20 @@ pow2_kernel(const __grid_constant__ PassDesc p)
 #pragma unroll
             for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], __ldg(twp + (unsigned)DOP_KL(i) * tws));
         }
-        if (!COL && RL >= 2) {
+        if (STAGE) { // (the exchange buffer is free: the last exchange ended with a __syncthreads)
+            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * (32 * STG_LANE);
+            const int lane = tid & 31;
+            char* g0 = reinterpret_cast<char*>(p.field + bL - lane * 16);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                *reinterpret_cast<float4*>(wb + lane * STG_LANE + j * 16) =
+                    make_float4(v[2 * j].x, v[2 * j].y, v[2 * j + 1].x, v[2 * j + 1].y);
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                *reinterpret_cast<float4*>(g0 + j * 512 + lane * 16) =
+                    *reinterpret_cast<const float4*>(wb + (4 * j + (lane >> 3)) * STG_LANE + (lane & 7) * 16);
+        } else if (!COL && RL >= 2) {
 #pragma unroll
             for (int i = 0; i < P; i += 2)
                 *reinterpret_cast<float4*>(p.field + bL + DOP_KL(i)) = make_float4(v[i].x, v[i].y, v[i + 1].x, v[i + 1].y);
@@ -533,7 +569,9 @@ static cudaError_t launch_one(const PassDesc& p, cudaStream_t stream)
 {
     using TL = fx::Tile<L, COL>;
     constexpr int threads = tile_threads(L, COL);
-    constexpr int smem = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
+    constexpr int smem_x = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
+    constexpr int smem_stage = COL ? 0 : (threads / 32) * 32 * (16 * 8 + 16); // per-warp staging (row tiles, RL = 16)
+    constexpr int smem = smem_x > smem_stage ? smem_x : smem_stage;
     static bool attr_done = false; // per instantiation; the attribute is per device function
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
