@@ -197,18 +197,18 @@ __host__ __device__ constexpr int group_freq(int c)
 
 // ---- tile-level engine --------------------------------------------------------------------------
 // Shared-memory layout of one tile.
-//   COL = true : NB = 16 adjacent lines; element (slot, col) at slot*16 + col (conflict-free).
+//   COL = true : NB (16, 32 or 64) adjacent lines; element (slot, col) at slot*NB + col (conflict-free).
 //   COL = false: one line; slot s at s + 2*(s >> 5) (two pad elements per 32 keep every access
 //                pattern of the schedule conflict-free and 16-byte alignment of even slots).
-template <int L, bool COL>
+template <int L, bool COL, int NB = 16>
 struct Tile {
     using S = Sched<L>;
     static constexpr int T = L / P;                                   // threads per line
-    static constexpr int LINE_ELEMS = COL ? L * 16 : L + 2 * (L / 32); // float2 per tile (COL) / line (row)
+    static constexpr int LINE_ELEMS = COL ? L * NB : L + 2 * (L / 32); // float2 per tile (COL) / line (row)
 
     __device__ static __forceinline__ int addr(int slot, int off)
     {
-        return COL ? (slot << 4) + off : slot + ((slot >> 5) << 1) + off;
+        return COL ? slot * NB + off : slot + ((slot >> 5) << 1) + off;
     }
     // slot of register i in the layout of group G
     template <int G>

@@ -1,5 +1,7 @@
 // kernels_pow2.cu -- dispatcher of the register-blocked power-of-two tile-pass kernels
 // (pow2_impl.cuh; instantiated per digit length in pow2_inst.cu) and their host-side tables.
+#include <cstdlib>
+
 #include "pow2_impl.cuh"
 
 namespace dop {
@@ -25,7 +27,23 @@ bool pow2_supported(long long L, bool col_type)
     return col_type ? L <= 512 : (L >= 64 && L <= 8192);
 }
 
-int pow2_lines(long long L, bool col_type) { return col_type ? 16 : row_lines((int)L); }
+// Lines per tile.  Column tiles: the bundle width NB.  `plain_y` = a non-last y digit (plain
+// forward / inverse passes only): measured on B200 (C4, L = 256) 32-column bundles (256-byte
+// segments, 512-thread CTAs) take the plain y passes from 0.67 to 0.75 of the measured copy
+// bandwidth, but cost the register-heavy fused variants 15-30 %, so only those digits get them.
+// DOP_COL_NB = 16 | 32 | 64 overrides for every column tile (clamped to what is instantiated).
+int pow2_lines(long long L, bool col_type, bool plain_y)
+{
+    if (!col_type) return row_lines((int)L);
+    if (L % 3 == 0) return 16;
+    int nb = (plain_y && L >= 256) ? 32 : 16;
+    if (const char* e = std::getenv("DOP_COL_NB")) {
+        const int v = std::atoi(e);
+        if (v == 16 || v == 32 || v == 64) nb = v;
+    }
+    const int mx = max_col_nb((int)L);
+    return nb < mx ? nb : mx;
+}
 
 // which fused-op variant a pass is, or -1 if the fast kernels do not implement the combination
 static int pass_variant(const PassDesc& p)
@@ -53,7 +71,8 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
     *handled = false;
     const bool col = p.col_type != 0;
     if (p.tw_g == nullptr || !pow2_supported(p.L, col)) return cudaSuccess;
-    if (p.nl != pow2_lines(p.L, col) || p.NC % p.nl != 0) return cudaSuccess;
+    if (col ? !(p.nl == 16 || p.nl == 32 || p.nl == 64) : p.nl != pow2_lines(p.L, false)) return cudaSuccess;
+    if (p.NC % p.nl != 0) return cudaSuccess;
     const int v = pass_variant(p);
     if (v < 0) return cudaSuccess;
     if ((v == V_H || v == V_GAUSS) && (!col || p.row_i != 1)) return cudaSuccess;

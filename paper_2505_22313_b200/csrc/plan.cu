@@ -139,7 +139,7 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         // column-type unless it is the last x digit
         const bool col_type = !(a == 0 && d.st == 1);
         const long long lines = col_type ? (a == 0 ? d.st : p->desc.nx) : p->desc.ny * (N / d.L);
-        d.fast = !p->force_generic && pow2_supported(d.L, col_type) && lines % pow2_lines(d.L, col_type) == 0;
+        d.fast = !p->force_generic && pow2_supported(d.L, col_type) && lines % pow2_lines(d.L, col_type, a == 1 && d.has_twb) == 0;
         if (d.fast) d.twg = pow2_group_twiddles(d.L);
         if (d.fast && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
             const long long Nj = d.L * d.st;
@@ -254,7 +254,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
         d->n_m = nx / (L * st); d->SM = L * st;
         d->n_o = ny; d->SO = nx;
         d->r_from = 0;
-        d->nl = fast ? 16 : (int)std::min<long long>(std::max<long long>(nl_target, 16), st);
+        d->nl = fast ? pow2_lines(L, true) : (int)std::min<long long>(std::max<long long>(nl_target, 16), st);
     } else { // y digit: lines are adjacent columns, elements st rows apart
         d->col_type = 1;
         d->es = st * nx;
@@ -263,7 +263,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
         d->n_o = ny / (L * st); d->SO = L * st * nx;
         d->r_from = 1;
         d->row_o = L * st; d->row_m = 1; d->row_i = st;
-        d->nl = fast ? 16 : (int)std::min<long long>(std::max<long long>(nl_target, 16), nx);
+        d->nl = fast ? pow2_lines(L, true, g.has_twb) : (int)std::min<long long>(std::max<long long>(nl_target, 16), nx);
     }
     d->n_cgroups = (d->NC + d->nl - 1) / d->nl;
     d->smem_bytes = (int)((long long)d->nl * L * (long long)sizeof(float2));

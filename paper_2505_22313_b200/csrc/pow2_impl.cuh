@@ -43,7 +43,7 @@ __host__ __device__ constexpr int variant_dir1(int v)
 __host__ __device__ constexpr int variant_dir2(int v) { return v == V_LOSS ? +1 : (v == V_H || v == V_GAUSS) ? -1 : 0; }
 
 __host__ __device__ constexpr int row_lines(int L) { return L >= 4096 ? 1 : 4096 / L; }
-__host__ __device__ constexpr int tile_threads(int L, bool col) { return col ? L : row_lines(L) * (L / P); }
+__host__ __device__ constexpr int tile_threads(int L, bool col, int nb = 16) { return col ? nb * (L / P) : row_lines(L) * (L / P); }
 // resident CTAs per SM the register allocation is asked to allow
 #ifndef DOP_RESIDENT_THREADS
 #define DOP_RESIDENT_THREADS 1024 // 65536 regs / 1024 threads -> 64 registers per thread (measured best: 768 -> 1024 gave C4 +10%)
@@ -54,10 +54,11 @@ __host__ __device__ constexpr int tile_threads(int L, bool col) { return col ? L
 #ifndef DOP_HEAVY_THREADS
 #define DOP_HEAVY_THREADS DOP_RESIDENT_THREADS // register budget of the loss / H / Gaussian variants
 #endif
-__host__ __device__ constexpr int min_blocks(int L, bool col, int v = 0)
+__host__ __device__ constexpr int min_blocks(int L, bool col, int v = 0, int nb = 16)
 {
     const int rt = v == 2 ? DOP_LOSS_THREADS : (v == 3 || v == 4) ? DOP_HEAVY_THREADS : DOP_RESIDENT_THREADS;
-    return tile_threads(L, col) >= 512 ? 2 : (rt / tile_threads(L, col) > 0 ? rt / tile_threads(L, col) : 1);
+    const int th = tile_threads(L, col, nb);
+    return th >= 512 ? (th >= 1024 ? 1 : 2) : (rt / th > 0 ? rt / th : 1);
 }
 
 // Cache-hinted global accesses as plain (non-volatile) asm so the unrolled loads can be scheduled
@@ -94,12 +95,16 @@ __device__ __forceinline__ void prefetch_tile(const PassDesc& p, int slots_per_t
     const long long o = (long long)(t / nm) + p.o0;
     const long long base = o * p.SO + m * p.SM + cg * NLINES * p.SCc;
     const int tid = threadIdx.x;
-    if (COL) { // slot tid (+ k THREADS): 16 adjacent columns = one 128-byte line of the field
+    if (COL) { // NLINES adjacent columns of one slot = NLINES/16 lines of the field, one per thread
+        constexpr int PER = NLINES / 16;
+        const int piece = tid % PER;
         for (int k = 0; k < slots_per_thread; ++k) {
-            const long long off = base + (long long)(tid + k * THREADS) * p.es;
-            if (WANT_FIELD) prefetch_l2(p.field + off);
-            if (WANT_HEIGHT) prefetch_l2(p.height + off);
-            if (WANT_PLANE) prefetch_l2(p.plane_in + off);
+            const long long off = base + (long long)(tid / PER + k * (THREADS / PER)) * p.es;
+            if (WANT_FIELD) prefetch_l2(p.field + off + piece * 16);
+            if (piece * 32 < NLINES) {
+                if (WANT_HEIGHT) prefetch_l2(p.height + off + piece * 32);
+                if (WANT_PLANE) prefetch_l2(p.plane_in + off + piece * 32);
+            }
         }
     } else { // the tile is NLINES * L contiguous points = THREADS lines of 16 complex64
         const long long off = base + (long long)tid * 16;
@@ -186,11 +191,11 @@ __device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double f
 }
 
 // ---- the tile-pass kernel -------------------------------------------------------------------
-template <int L, bool COL, int V, int TWB>
-__global__ void __launch_bounds__(tile_threads(L, COL), min_blocks(L, COL, V))
+template <int L, bool COL, int V, int TWB, int NB>
+__global__ void __launch_bounds__(tile_threads(L, COL, NB), min_blocks(L, COL, V, NB))
 pow2_kernel(const __grid_constant__ PassDesc p)
 {
-    using TL = fx::Tile<L, COL>;
+    using TL = fx::Tile<L, COL, NB>;
     using S = fx::Sched<L>;
     constexpr int T = L / P;            // threads per line
     constexpr int GL = S::NG - 1;       // last group
@@ -218,9 +223,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     const long long m = t % nm;
     const long long o = (long long)(t / nm) + p.o0;
     const int tid = threadIdx.x;
-    const int sub = COL ? (tid & 15) : (tid / T); // column in the bundle / line in the tile
-    const int tt = COL ? (tid >> 4) : (tid % T);
-    const long long line = cg * (COL ? 16 : LINES) + sub;
+    const int sub = COL ? (tid % NB) : (tid / T); // column in the bundle / line in the tile
+    const int tt = COL ? (tid / NB) : (tid % T);
+    const long long line = cg * (COL ? NB : LINES) + sub;
     const long long es = COL ? p.es : 1;
     const long long tbase = o * p.SO + m * p.SM + line * p.SCc;
     const int soff = COL ? sub : sub * TL::LINE_ELEMS;
@@ -251,7 +256,7 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     // (not compiled into the x column tiles: it never pays there and its registers cost the loss
     // variant 25%, C4 32 -> 41 ms)
     if (!COL || TWB != TWB_LANE)
-        prefetch_tile<COL, tile_threads(L, COL), COL ? 16 : LINES, (V != V_HEIGHT && V != V_LDOTHER),
+        prefetch_tile<COL, tile_threads(L, COL, NB), COL ? NB : LINES, (V != V_HEIGHT && V != V_LDOTHER),
                       (V == V_HEIGHT || V == V_GRAD), (V == V_LOSS)>(p, 1, L);
 
     // Touch the tables this tile will need after its DFT now, so they are in L1 by then.
@@ -364,7 +369,7 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         __syncthreads();
         if (tid == 0) {
             double r = 0.0;
-            constexpr int NW = (tile_threads(L, COL) + 31) / 32;
+            constexpr int NW = (tile_threads(L, COL, NB) + 31) / 32;
             for (int w = 0; w < NW; ++w) r += red[w];
             p.loss_scratch[p.tile0 + blockIdx.x] = r;
         }
@@ -564,27 +569,57 @@ cudaError_t launch_x3(const PassDesc& p, int variant, int twb, cudaStream_t st)
 }
 
 // ---- host side -------------------------------------------------------------------------------
-template <int L, bool COL, int V, int TWB>
+template <int L, bool COL, int V, int TWB, int NB = 16>
 static cudaError_t launch_one(const PassDesc& p, cudaStream_t stream)
 {
-    using TL = fx::Tile<L, COL>;
-    constexpr int threads = tile_threads(L, COL);
+    using TL = fx::Tile<L, COL, NB>;
+    constexpr int threads = tile_threads(L, COL, NB);
     constexpr int smem_x = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
     constexpr int smem_stage = COL ? 0 : (threads / 32) * 32 * (16 * 8 + 16); // per-warp staging (row tiles, RL = 16)
     constexpr int smem = smem_x > smem_stage ? smem_x : smem_stage;
     static bool attr_done = false; // per instantiation; the attribute is per device function
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB>, cudaFuncAttributePreferredSharedMemoryCarveout,
+        e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB, NB>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                  cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
     if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
-    pow2_kernel<L, COL, V, TWB><<<(unsigned)ntiles, threads, smem, stream>>>(p);
+    pow2_kernel<L, COL, V, TWB, NB><<<(unsigned)ntiles, threads, smem, stream>>>(p);
     return cudaGetLastError();
+}
+
+// All variants of one (L, tile type).  Returns cudaErrorInvalidValue for a combination that is
+// never scheduled (the dispatcher then falls back to the generic kernel).
+// widest column bundle instantiated for a digit length: 64 columns up to L = 128, 32 up to 256
+__host__ __device__ constexpr int max_col_nb(int L) { return L <= 128 ? 64 : (L <= 256 ? 32 : 16); }
+
+template <int L, int NB>
+cudaError_t launch_col(const PassDesc& p, int variant, int twb, cudaStream_t st)
+{
+    if constexpr (NB <= max_col_nb(L)) {
+        if (twb == TWB_NONE) {
+            if (variant == V_H) return launch_one<L, true, V_H, TWB_NONE, NB>(p, st);
+            if (variant == V_GAUSS) return launch_one<L, true, V_GAUSS, TWB_NONE, NB>(p, st);
+        } else if (twb == TWB_TILE) {
+            if (variant == V_FWD) return launch_one<L, true, V_FWD, TWB_TILE, NB>(p, st);
+            if (variant == V_INV) return launch_one<L, true, V_INV, TWB_TILE, NB>(p, st);
+        } else {
+            switch (variant) {
+            case V_FWD: return launch_one<L, true, V_FWD, TWB_LANE, NB>(p, st);
+            case V_INV: return launch_one<L, true, V_INV, TWB_LANE, NB>(p, st);
+            case V_LOSS: return launch_one<L, true, V_LOSS, TWB_LANE, NB>(p, st);
+            case V_HEIGHT: return launch_one<L, true, V_HEIGHT, TWB_LANE, NB>(p, st);
+            case V_LDOTHER: return launch_one<L, true, V_LDOTHER, TWB_LANE, NB>(p, st);
+            case V_GRAD: return launch_one<L, true, V_GRAD, TWB_LANE, NB>(p, st);
+            case V_STOTHER: return launch_one<L, true, V_STOTHER, TWB_LANE, NB>(p, st);
+            }
+        }
+    }
+    return cudaErrorInvalidValue;
 }
 
 // All variants of one (L, tile type).  Returns cudaErrorInvalidValue for a combination that is
@@ -593,23 +628,9 @@ template <int L, bool COL>
 cudaError_t launch_L(const PassDesc& p, int variant, int twb, cudaStream_t st)
 {
     if constexpr (COL) {
-        if (twb == TWB_NONE) {
-            if (variant == V_H) return launch_one<L, true, V_H, TWB_NONE>(p, st);
-            if (variant == V_GAUSS) return launch_one<L, true, V_GAUSS, TWB_NONE>(p, st);
-        } else if (twb == TWB_TILE) {
-            if (variant == V_FWD) return launch_one<L, true, V_FWD, TWB_TILE>(p, st);
-            if (variant == V_INV) return launch_one<L, true, V_INV, TWB_TILE>(p, st);
-        } else {
-            switch (variant) {
-            case V_FWD: return launch_one<L, true, V_FWD, TWB_LANE>(p, st);
-            case V_INV: return launch_one<L, true, V_INV, TWB_LANE>(p, st);
-            case V_LOSS: return launch_one<L, true, V_LOSS, TWB_LANE>(p, st);
-            case V_HEIGHT: return launch_one<L, true, V_HEIGHT, TWB_LANE>(p, st);
-            case V_LDOTHER: return launch_one<L, true, V_LDOTHER, TWB_LANE>(p, st);
-            case V_GRAD: return launch_one<L, true, V_GRAD, TWB_LANE>(p, st);
-            case V_STOTHER: return launch_one<L, true, V_STOTHER, TWB_LANE>(p, st);
-            }
-        }
+        if (p.nl == 16) return launch_col<L, 16>(p, variant, twb, st);
+        if (p.nl == 32) return launch_col<L, 32>(p, variant, twb, st);
+        if (p.nl == 64) return launch_col<L, 64>(p, variant, twb, st);
     } else {
         if (twb == TWB_NONE) {
             switch (variant) {
