@@ -206,12 +206,15 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     // L2-only field accesses: column tiles except the two variants where it measured slower (C4:
     // loss pass 32 -> 45 ms, height pass 12.5 -> 13.7 ms)
     constexpr bool CG = COL && V != V_LOSS && V != V_HEIGHT;
-    // Row tiles whose last group is radix 16: a thread owns 16 adjacent slots (128 bytes) and a warp 4 KiB of
-    // contiguous memory.  Its global accesses are staged through a padded per-warp shared-memory
-    // buffer so that every LDG/STG.128 of the warp covers 512 contiguous bytes instead of 16 bytes
-    // in each of 32 lines.
-    constexpr bool STAGE = !COL && RL == 16;
-    constexpr int STG_LANE = 16 * 8 + 16; // bytes per lane: 128 + 16 padding (conflict-free both ways)
+    // Row tiles whose last group has radix >= 4: a thread owns runs of RL adjacent slots, so its own
+    // 16-byte accesses would touch 32 different lines per warp instruction.  The warp's 4 KiB are
+    // staged through a padded per-warp shared-memory buffer instead, so that every LDG/STG.128 of
+    // the warp covers 512 contiguous bytes (x passes at C4: 0.61 / 0.72 -> 0.88 / 0.99 of measured
+    // copy bandwidth).  Footprint of a warp: T < 32: 32/T whole lines, contiguous; T >= 32: P/RL chunks
+    // of 32 runs each, T RL slots apart.
+    constexpr bool STAGE = !COL && RL >= 4;
+    constexpr int STG_WARP = 4096 + 32 * 16; // bytes per warp: 4 KiB + 16 bytes of padding per 128
+    constexpr int CHUNK = 32 * RL * 8;        // T >= 32: bytes of one run index across the warp
     extern __shared__ float2 s[];
 
     // ---- which tile (same enumeration as the generic kernel)
@@ -242,6 +245,17 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     const long long step0 = (long long)T * es;                  // first-group layout: register i -> i + 1
     const long long stepLr = (long long)(T * RL - (RL - 1)) * es; // last-group layout: end of a run of RL -> next run
 #define DOP_NEXT_L(ptr, i) ptr += ((((i) % RL) == RL - 1) ? stepLr : es)
+
+    // staging geometry (row tiles): linear position of this lane's register pair (2q, 2q+1) in the warp's
+    // footprint, global byte offset of a linear position, padded shared-memory address
+    const int lane = tid & 31;
+#define DOP_STG_OWN(q) (T >= 32 ? ((2 * (q)) / RL) * CHUNK + lane * (RL * 8) + ((2 * (q)) % RL) * 8 \
+                                : (lane / (T >= 32 ? 1 : T)) * (L * 8) + ((2 * (q)) / RL) * (T * RL * 8) + \
+                                      (lane % (T >= 32 ? 1 : T)) * (RL * 8) + ((2 * (q)) % RL) * 8)
+#define DOP_STG_GLOB(x) (T >= 32 ? ((x) / CHUNK) * (T * RL * 8) + (x) % CHUNK : (x))
+#define DOP_STG_PAD(x) ((x) + (((x) >> 7) << 4))
+    const long long stg_base = bL - (T >= 32 ? (long long)lane * RL
+                                             : (long long)(lane / (T >= 32 ? 1 : T)) * L + (lane % (T >= 32 ? 1 : T)) * RL);
 
     // boundary twiddle of the element in register i (last-group layout)
     const float2* __restrict__ twp = nullptr;
@@ -293,20 +307,20 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         }
     } else {
         if (STAGE) {
-            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * (32 * STG_LANE);
-            const int lane = tid & 31;
-            const char* g0 = reinterpret_cast<const char*>(p.field + bL - lane * 16); // the warp's 4 KiB
+            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * STG_WARP;
+            const char* g0 = reinterpret_cast<const char*>(p.field + stg_base); // the warp's footprint
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const float4 q = *reinterpret_cast<const float4*>(g0 + j * 512 + lane * 16);
-                *reinterpret_cast<float4*>(wb + (4 * j + (lane >> 3)) * STG_LANE + (lane & 7) * 16) = q;
+                const int x = j * 512 + lane * 16;
+                *reinterpret_cast<float4*>(wb + DOP_STG_PAD(x)) = *reinterpret_cast<const float4*>(g0 + DOP_STG_GLOB(x));
             }
             __syncwarp();
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const float4 q = *reinterpret_cast<const float4*>(wb + lane * STG_LANE + j * 16);
-                v[2 * j] = make_float2(q.x, q.y);
-                v[2 * j + 1] = make_float2(q.z, q.w);
+            for (int q = 0; q < 8; ++q) {
+                const int x = DOP_STG_OWN(q);
+                const float4 w = *reinterpret_cast<const float4*>(wb + DOP_STG_PAD(x));
+                v[2 * q] = make_float2(w.x, w.y);
+                v[2 * q + 1] = make_float2(w.z, w.w);
             }
             __syncthreads(); // the staging area overlaps the exchange buffer of the DFT below
         } else if (!COL && RL >= 2) {
@@ -385,18 +399,19 @@ pow2_kernel(const __grid_constant__ PassDesc p)
             for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], __ldg(twp + (unsigned)DOP_KL(i) * tws));
         }
         if (STAGE) { // (the exchange buffer is free: the last exchange ended with a __syncthreads)
-            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * (32 * STG_LANE);
-            const int lane = tid & 31;
-            char* g0 = reinterpret_cast<char*>(p.field + bL - lane * 16);
+            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * STG_WARP;
+            char* g0 = reinterpret_cast<char*>(p.field + stg_base);
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-                *reinterpret_cast<float4*>(wb + lane * STG_LANE + j * 16) =
-                    make_float4(v[2 * j].x, v[2 * j].y, v[2 * j + 1].x, v[2 * j + 1].y);
+            for (int q = 0; q < 8; ++q) {
+                const int x = DOP_STG_OWN(q);
+                *reinterpret_cast<float4*>(wb + DOP_STG_PAD(x)) = make_float4(v[2 * q].x, v[2 * q].y, v[2 * q + 1].x, v[2 * q + 1].y);
+            }
             __syncwarp();
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-                *reinterpret_cast<float4*>(g0 + j * 512 + lane * 16) =
-                    *reinterpret_cast<const float4*>(wb + (4 * j + (lane >> 3)) * STG_LANE + (lane & 7) * 16);
+            for (int j = 0; j < 8; ++j) {
+                const int x = j * 512 + lane * 16;
+                *reinterpret_cast<float4*>(g0 + DOP_STG_GLOB(x)) = *reinterpret_cast<const float4*>(wb + DOP_STG_PAD(x));
+            }
         } else if (!COL && RL >= 2) {
 #pragma unroll
             for (int i = 0; i < P; i += 2)
@@ -435,6 +450,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
 #undef DOP_K0
 #undef DOP_KL
 #undef DOP_NEXT_L
+#undef DOP_STG_OWN
+#undef DOP_STG_GLOB
+#undef DOP_STG_PAD
 }
 
 // ---- digits of length 3 * 2^k: one radix-3 step fused in front of three register-blocked 2^k DFTs
@@ -575,7 +593,7 @@ static cudaError_t launch_one(const PassDesc& p, cudaStream_t stream)
     using TL = fx::Tile<L, COL, NB>;
     constexpr int threads = tile_threads(L, COL, NB);
     constexpr int smem_x = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
-    constexpr int smem_stage = COL ? 0 : (threads / 32) * 32 * (16 * 8 + 16); // per-warp staging (row tiles, RL = 16)
+    constexpr int smem_stage = COL ? 0 : (threads / 32) * (4096 + 32 * 16); // per-warp staging (row tiles)
     constexpr int smem = smem_x > smem_stage ? smem_x : smem_stage;
     static bool attr_done = false; // per instantiation; the attribute is per device function
     if (!attr_done) {
