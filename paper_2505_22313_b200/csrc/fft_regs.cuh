@@ -219,17 +219,44 @@ struct Tile {
         const int bf = tt + u * T;
         return (bf & ~(m - 1)) * R + (bf & (m - 1)) + c * m;
     }
+    // Shared-memory address of register i in the layout of group G, split into a per-thread base (one
+    // per butterfly u = i / R) and a compile-time offset (c = i % R), so that the 16 accesses of an
+    // exchange use immediate offsets.  The row padding is separable: the butterfly's base slot is a
+    // multiple of R m or has its low part < m, and m | 32, so ((base + c m) >> 5) = (base >> 5) + ((c m) >> 5).
+    template <int G>
+    __device__ static __forceinline__ int base_addr(int tt, int u, int off)
+    {
+        constexpr int R = S::radix(G), m = S::block(G) / R;
+        const int bf = tt + u * T;
+        return addr((bf & ~(m - 1)) * R + (bf & (m - 1)), off);
+    }
+    template <int G>
+    __host__ __device__ static constexpr int reg_offset(int c)
+    {
+        constexpr int R = S::radix(G), m = S::block(G) / R;
+        return COL ? c * m * NB : c * m + (((c * m) >> 5) << 1);
+    }
     template <int G>
     __device__ static __forceinline__ void to_smem(const float2* v, float2* s, int tt, int off)
     {
+        constexpr int R = S::radix(G);
 #pragma unroll
-        for (int i = 0; i < P; ++i) s[addr(slot<G>(tt, i), off)] = v[i];
+        for (int u = 0; u < P / R; ++u) {
+            float2* b = s + base_addr<G>(tt, u, off);
+#pragma unroll
+            for (int c = 0; c < R; ++c) b[reg_offset<G>(c)] = v[u * R + c];
+        }
     }
     template <int G>
     __device__ static __forceinline__ void from_smem(float2* v, const float2* s, int tt, int off)
     {
+        constexpr int R = S::radix(G);
 #pragma unroll
-        for (int i = 0; i < P; ++i) v[i] = s[addr(slot<G>(tt, i), off)];
+        for (int u = 0; u < P / R; ++u) {
+            const float2* b = s + base_addr<G>(tt, u, off);
+#pragma unroll
+            for (int c = 0; c < R; ++c) v[u * R + c] = b[reg_offset<G>(c)];
+        }
     }
     template <int G, int DIR>
     __device__ static __forceinline__ void butterflies(float2* v, int tt, const float2* __restrict__ tw)
