@@ -210,13 +210,30 @@ struct Tile {
     {
         return COL ? slot * NB + off : slot + ((slot >> 5) << 1) + off;
     }
+    // Butterfly handled by thread tt as its u-th one in group G.  Radix-16 groups: one butterfly per
+    // thread, bf = tt.  The remainder group (radix R < 16, always last, m = 1) has P/R per thread:
+    //   CONTIG  : consecutive ones, so that in the last group's layout a thread owns the 16 adjacent
+    //             slots 16 tt .. 16 tt + 15: its exchange with the previous group stays inside that
+    //             group's block (warp-local when the block has <= 512 slots), and global accesses
+    //             are 128-byte runs that the row kernels stage through shared memory;
+    //   !CONTIG : T apart (runs of R slots).  Kept for row tiles with R = 2 (L = 512, 8192), whose
+    //             16-byte runs are already perfectly coalesced straight from registers (staging
+    //             measured 15 % slower there), and for column tiles (no staging; L = 64 measured
+    //             10 % slower with the consecutive assignment).
+    static constexpr bool CONTIG = !COL && S::RLAST != 2;
+    template <int G>
+    __device__ static __forceinline__ int bfly(int tt, int u)
+    {
+        constexpr int R = S::radix(G);
+        return (CONTIG && P / R > 1) ? tt * (P / R) + u : tt + u * T;
+    }
     // slot of register i in the layout of group G
     template <int G>
     __device__ static __forceinline__ int slot(int tt, int i)
     {
         constexpr int R = S::radix(G), m = S::block(G) / R;
         const int u = i / R, c = i % R;
-        const int bf = tt + u * T;
+        const int bf = bfly<G>(tt, u);
         return (bf & ~(m - 1)) * R + (bf & (m - 1)) + c * m;
     }
     // Shared-memory address of register i in the layout of group G, split into a per-thread base (one
@@ -227,7 +244,7 @@ struct Tile {
     __device__ static __forceinline__ int base_addr(int tt, int u, int off)
     {
         constexpr int R = S::radix(G), m = S::block(G) / R;
-        const int bf = tt + u * T;
+        const int bf = bfly<G>(tt, u);
         return addr((bf & ~(m - 1)) * R + (bf & (m - 1)), off);
     }
     template <int G>
@@ -265,7 +282,7 @@ struct Tile {
 #pragma unroll
         for (int u = 0; u < P / R; ++u) {
             float2* w = v + u * R;
-            const int j = (tt + u * T) & (m - 1);
+            const int j = bfly<G>(tt, u) & (m - 1);
             if (DIR < 0 && m > 1) {
 #pragma unroll
                 for (int c = 1; c < R; ++c)
@@ -279,30 +296,50 @@ struct Tile {
             }
         }
     }
+    // An exchange between groups GA and GB only moves data inside blocks of block(min(GA, GB)) slots,
+    // i.e. among block/16 consecutive threads of a row tile: at most one warp when block <= 512.  Such
+    // exchanges need __syncwarp() only; a CTA-wide one additionally needs a leading __syncthreads()
+    // when the previous shared-memory activity was only warp-synchronised (PREV_WIDE = false).
+    template <int GA, int GB>
+    __host__ __device__ static constexpr bool local_exchange()
+    {
+        return !COL && S::block(GA < GB ? GA : GB) / P <= 32 &&
+               (CONTIG || (S::radix(GA) == 16 && S::radix(GB) == 16));
+    }
+    template <bool LOCAL>
+    __device__ static __forceinline__ void xsync()
+    {
+        if (LOCAL) __syncwarp();
+        else __syncthreads();
+    }
     // forward: v in the layout of group 0  ->  v in the layout of the last group
-    template <int G = 0>
+    template <int G = 0, bool PREV_WIDE = COL>
     __device__ static __forceinline__ void forward(float2* v, float2* s, int tt, int off, const float2* __restrict__ tw)
     {
         butterflies<G, +1>(v, tt, tw);
         if constexpr (G + 1 < S::NG) {
+            constexpr bool loc = local_exchange<G, G + 1>();
+            if (!loc && !PREV_WIDE) __syncthreads();
             to_smem<G>(v, s, tt, off);
-            __syncthreads();
+            xsync<loc>();
             from_smem<G + 1>(v, s, tt, off);
-            __syncthreads();
-            forward<G + 1>(v, s, tt, off, tw);
+            xsync<loc>();
+            forward<G + 1, !loc>(v, s, tt, off, tw);
         }
     }
     // inverse (unnormalised): v in the layout of the last group  ->  layout of group 0
-    template <int G = S::NG - 1>
+    template <int G = S::NG - 1, bool PREV_WIDE = COL>
     __device__ static __forceinline__ void inverse(float2* v, float2* s, int tt, int off, const float2* __restrict__ tw)
     {
         butterflies<G, -1>(v, tt, tw);
         if constexpr (G > 0) {
+            constexpr bool loc = local_exchange<G, G - 1>();
+            if (!loc && !PREV_WIDE) __syncthreads();
             to_smem<G>(v, s, tt, off);
-            __syncthreads();
+            xsync<loc>();
             from_smem<G - 1>(v, s, tt, off);
-            __syncthreads();
-            inverse<G - 1>(v, s, tt, off, tw);
+            xsync<loc>();
+            inverse<G - 1, !loc>(v, s, tt, off, tw);
         }
     }
 };

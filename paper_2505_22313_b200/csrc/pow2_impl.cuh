@@ -199,22 +199,21 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     using S = fx::Sched<L>;
     constexpr int T = L / P;            // threads per line
     constexpr int GL = S::NG - 1;       // last group
-    constexpr int RL = S::radix(GL);    // its radix
+    constexpr int RL = TL::CONTIG ? P : S::radix(GL); // adjacent slots per run in the last group's layout (fft_regs.cuh bfly)
     constexpr int DIR1 = variant_dir1(V), DIR2 = variant_dir2(V);
     constexpr int LAST = DIR2 != 0 ? DIR2 : DIR1;
     constexpr int LINES = row_lines(L);
     // L2-only field accesses: column tiles except the two variants where it measured slower (C4:
     // loss pass 32 -> 45 ms, height pass 12.5 -> 13.7 ms)
     constexpr bool CG = COL && V != V_LOSS && V != V_HEIGHT;
-    // Row tiles whose last group has radix >= 4: a thread owns runs of RL adjacent slots, so its own
-    // 16-byte accesses would touch 32 different lines per warp instruction.  The warp's 4 KiB are
-    // staged through a padded per-warp shared-memory buffer instead, so that every LDG/STG.128 of
-    // the warp covers 512 contiguous bytes (x passes at C4: 0.61 / 0.72 -> 0.88 / 0.99 of measured
-    // copy bandwidth).  Footprint of a warp: T < 32: 32/T whole lines, contiguous; T >= 32: P/RL chunks
-    // of 32 runs each, T RL slots apart.
-    constexpr bool STAGE = !COL && RL >= 4;
-    constexpr int STG_WARP = 4096 + 32 * 16; // bytes per warp: 4 KiB + 16 bytes of padding per 128
-    constexpr int CHUNK = 32 * RL * 8;        // T >= 32: bytes of one run index across the warp
+    // Row tiles: in the last group's layout a thread owns 16 adjacent slots (128 bytes) and a warp 512
+    // adjacent slots (4 KiB of contiguous memory: part of one line when T >= 32, 32/T whole lines
+    // otherwise).  Global accesses in that layout go through the exchange buffer: the warp moves its 4 KiB
+    // with LDG/STG.128 that each cover 512 contiguous bytes, and the threads pick up / drop their own
+    // 16 slots in shared memory (x passes at C4: 0.61 / 0.72 -> 0.88 / 0.99 of measured copy bandwidth
+    // against 16-byte accesses to 32 different lines per instruction).  Only the warp's own slots are
+    // touched, so the hazards are warp-local.
+    constexpr bool STAGE = !COL && TL::CONTIG; // (L = 512, 8192: runs of 2 slots, coalesced as they are)
     extern __shared__ float2 s[];
 
     // ---- which tile (same enumeration as the generic kernel)
@@ -246,16 +245,14 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     const long long stepLr = (long long)(T * RL - (RL - 1)) * es; // last-group layout: end of a run of RL -> next run
 #define DOP_NEXT_L(ptr, i) ptr += ((((i) % RL) == RL - 1) ? stepLr : es)
 
-    // staging geometry (row tiles): linear position of this lane's register pair (2q, 2q+1) in the warp's
-    // footprint, global byte offset of a linear position, padded shared-memory address
+    // staging geometry (row tiles): shared-memory index (float2 units) of element e (even, 0..510) of the
+    // warp's 512 slots, and the global offset of the warp's first slot
     const int lane = tid & 31;
-#define DOP_STG_OWN(q) (T >= 32 ? ((2 * (q)) / RL) * CHUNK + lane * (RL * 8) + ((2 * (q)) % RL) * 8 \
-                                : (lane / (T >= 32 ? 1 : T)) * (L * 8) + ((2 * (q)) / RL) * (T * RL * 8) + \
-                                      (lane % (T >= 32 ? 1 : T)) * (RL * 8) + ((2 * (q)) % RL) * 8)
-#define DOP_STG_GLOB(x) (T >= 32 ? ((x) / CHUNK) * (T * RL * 8) + (x) % CHUNK : (x))
-#define DOP_STG_PAD(x) ((x) + (((x) >> 7) << 4))
-    const long long stg_base = bL - (T >= 32 ? (long long)lane * RL
-                                             : (long long)(lane / (T >= 32 ? 1 : T)) * L + (lane % (T >= 32 ? 1 : T)) * RL);
+    auto stg_addr = [&](int e) -> int {
+        if (T >= 32) return soff + TL::addr((tt - lane) * P + e, 0);
+        return (sub - lane / (T >= 32 ? 1 : T) + e / L) * TL::LINE_ELEMS + TL::addr(e % L, 0);
+    };
+    const long long stg_base = bL - (long long)lane * P;
 
     // boundary twiddle of the element in register i (last-group layout)
     const float2* __restrict__ twp = nullptr;
@@ -307,27 +304,24 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         }
     } else {
         if (STAGE) {
-            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * STG_WARP;
-            const char* g0 = reinterpret_cast<const char*>(p.field + stg_base); // the warp's footprint
+            const float2* g0 = p.field + stg_base; // the warp's 512 slots
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const int x = j * 512 + lane * 16;
-                *reinterpret_cast<float4*>(wb + DOP_STG_PAD(x)) = *reinterpret_cast<const float4*>(g0 + DOP_STG_GLOB(x));
+                const int e = j * 64 + 2 * lane;
+                *reinterpret_cast<float4*>(s + stg_addr(e)) = *reinterpret_cast<const float4*>(g0 + e);
             }
             __syncwarp();
+            const float4* own = reinterpret_cast<const float4*>(s + soff + TL::addr(tt * P, 0));
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-                const int x = DOP_STG_OWN(q);
-                const float4 w = *reinterpret_cast<const float4*>(wb + DOP_STG_PAD(x));
+                const float4 w = own[q];
                 v[2 * q] = make_float2(w.x, w.y);
                 v[2 * q + 1] = make_float2(w.z, w.w);
             }
-            __syncthreads(); // the staging area overlaps the exchange buffer of the DFT below
-        } else if (!COL && RL >= 2) {
+            __syncwarp();
+        } else if (!COL) { // runs of RL = 2 slots: one float4 per lane, 512 contiguous bytes per warp instruction
 #pragma unroll
             for (int i = 0; i < P; i += 2) {
-                // default caching on purpose: a thread reads RL adjacent slots 16 bytes at a time, the
-                // rest of each 128-byte line is picked up from L1 by the following loads
                 const float4 q = *reinterpret_cast<const float4*>(p.field + bL + DOP_KL(i));
                 v[i] = make_float2(q.x, q.y);
                 v[i + 1] = make_float2(q.z, q.w);
@@ -346,8 +340,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         }
     }
 
-    if (DIR1 > 0) TL::template forward<0>(v, s, tt, soff, tw);
-    else TL::template inverse<GL>(v, s, tt, soff, tw);
+    // (PREV_WIDE: no shared-memory activity yet, or it ended with a CTA barrier)
+    if (DIR1 > 0) TL::template forward<0, true>(v, s, tt, soff, tw);
+    else TL::template inverse<GL, !STAGE>(v, s, tt, soff, tw);
 
     // ---- middle op
     if (V == V_H) { // registers hold spectrum slots in the last group's layout; this is the last y digit
@@ -389,8 +384,8 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         }
     }
 
-    if (DIR2 > 0) TL::template forward<0>(v, s, tt, soff, tw);
-    else if (DIR2 < 0) TL::template inverse<GL>(v, s, tt, soff, tw);
+    if (DIR2 > 0) TL::template forward<0, COL>(v, s, tt, soff, tw);
+    else if (DIR2 < 0) TL::template inverse<GL, COL>(v, s, tt, soff, tw);
 
     // ---- store (+ boundary twiddle after a forward DFT, + epilogue op)
     if (LAST > 0) {
@@ -398,21 +393,18 @@ pow2_kernel(const __grid_constant__ PassDesc p)
 #pragma unroll
             for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], __ldg(twp + (unsigned)DOP_KL(i) * tws));
         }
-        if (STAGE) { // (the exchange buffer is free: the last exchange ended with a __syncthreads)
-            char* wb = reinterpret_cast<char*>(s) + (tid >> 5) * STG_WARP;
-            char* g0 = reinterpret_cast<char*>(p.field + stg_base);
+        if (STAGE) { // (the last exchange of a row tile is warp-local and ended with a __syncwarp)
+            float4* own = reinterpret_cast<float4*>(s + soff + TL::addr(tt * P, 0));
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const int x = DOP_STG_OWN(q);
-                *reinterpret_cast<float4*>(wb + DOP_STG_PAD(x)) = make_float4(v[2 * q].x, v[2 * q].y, v[2 * q + 1].x, v[2 * q + 1].y);
-            }
+            for (int q = 0; q < 8; ++q) own[q] = make_float4(v[2 * q].x, v[2 * q].y, v[2 * q + 1].x, v[2 * q + 1].y);
             __syncwarp();
+            float2* g0 = p.field + stg_base;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const int x = j * 512 + lane * 16;
-                *reinterpret_cast<float4*>(g0 + DOP_STG_GLOB(x)) = *reinterpret_cast<const float4*>(wb + DOP_STG_PAD(x));
+                const int e = j * 64 + 2 * lane;
+                *reinterpret_cast<float4*>(g0 + e) = *reinterpret_cast<const float4*>(s + stg_addr(e));
             }
-        } else if (!COL && RL >= 2) {
+        } else if (!COL) {
 #pragma unroll
             for (int i = 0; i < P; i += 2)
                 *reinterpret_cast<float4*>(p.field + bL + DOP_KL(i)) = make_float4(v[i].x, v[i].y, v[i + 1].x, v[i + 1].y);
@@ -450,9 +442,6 @@ pow2_kernel(const __grid_constant__ PassDesc p)
 #undef DOP_K0
 #undef DOP_KL
 #undef DOP_NEXT_L
-#undef DOP_STG_OWN
-#undef DOP_STG_GLOB
-#undef DOP_STG_PAD
 }
 
 // ---- digits of length 3 * 2^k: one radix-3 step fused in front of three register-blocked 2^k DFTs
@@ -592,9 +581,7 @@ static cudaError_t launch_one(const PassDesc& p, cudaStream_t stream)
 {
     using TL = fx::Tile<L, COL, NB>;
     constexpr int threads = tile_threads(L, COL, NB);
-    constexpr int smem_x = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
-    constexpr int smem_stage = COL ? 0 : (threads / 32) * (4096 + 32 * 16); // per-warp staging (row tiles)
-    constexpr int smem = smem_x > smem_stage ? smem_x : smem_stage;
+    constexpr int smem = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
     static bool attr_done = false; // per instantiation; the attribute is per device function
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
