@@ -35,8 +35,11 @@ bool pow2_supported(long long L, bool col_type)
 int pow2_lines(long long L, bool col_type, bool plain_y)
 {
     if (!col_type) return row_lines((int)L);
-    if (L % 3 == 0) return 16;
     int nb = (plain_y && L >= 256) ? 32 : 16;
+    if (L % 3 == 0) { // 3 * 2^k digits: 16 or 32 columns
+        if (const char* e = std::getenv("DOP_COL_NB")) nb = std::atoi(e) == 32 ? 32 : (std::atoi(e) == 16 ? 16 : nb);
+        return nb;
+    }
     if (const char* e = std::getenv("DOP_COL_NB")) {
         const int v = std::atoi(e);
         if (v == 16 || v == 32 || v == 64) nb = v;

@@ -448,11 +448,11 @@ pow2_kernel(const __grid_constant__ PassDesc p)
 // Column-type tiles, plain forward / inverse passes only (the plan puts the factor 3 in a
 // non-last digit).  Slot order = the generic kernel's for the radix list (3, 4, 4, ...): slot
 // c LP + i' holds output k = c + 3 k'(i').  Each thread keeps the three sub-tiles (48 points).
-template <int LP, int V, int TWB>
-__global__ void __launch_bounds__(LP, (512 / LP) > 0 ? (512 / LP) : 1)
+template <int LP, int V, int TWB, int NB>
+__global__ void __launch_bounds__(NB * (LP / P), (512 / (NB * (LP / P))) > 0 ? (512 / (NB * (LP / P))) : 1)
 pow2x3_kernel(const __grid_constant__ PassDesc p)
 {
-    using TL = fx::Tile<LP, true>;
+    using TL = fx::Tile<LP, true, NB>;
     using S = fx::Sched<LP>;
     constexpr int T = LP / P;
     constexpr int GL = S::NG - 1;
@@ -468,8 +468,8 @@ pow2x3_kernel(const __grid_constant__ PassDesc p)
     const long long m = t % nm;
     const long long o = (long long)(t / nm) + p.o0;
     const int tid = threadIdx.x;
-    const int sub = tid & 15, tt = tid >> 4;
-    const long long line = cg * 16 + sub;
+    const int sub = tid % NB, tt = tid / NB;
+    const long long line = cg * NB + sub;
     const long long es = p.es;
     const long long tbase = o * p.SO + m * p.SM + line * p.SCc;
     const float2* __restrict__ tw = p.tw_g;
@@ -485,7 +485,7 @@ pow2x3_kernel(const __grid_constant__ PassDesc p)
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
 
-    prefetch_tile<true, LP, 16, true, false, false>(p, 3, 3 * LP);
+    prefetch_tile<true, NB * (LP / P), NB, true, false, false>(p, 3, 3 * LP);
 
     float2 v[3][P];
     if (DIR > 0) {
@@ -546,32 +546,40 @@ pow2x3_kernel(const __grid_constant__ PassDesc p)
 #undef DOP_KL
 }
 
-template <int LP, int V, int TWB>
+template <int LP, int V, int TWB, int NB>
 static cudaError_t launch_x3_one(const PassDesc& p, cudaStream_t stream)
 {
-    constexpr int smem = fx::Tile<LP, true>::LINE_ELEMS * (int)sizeof(float2);
+    constexpr int smem = fx::Tile<LP, true, NB>::LINE_ELEMS * (int)sizeof(float2);
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(pow2x3_kernel<LP, V, TWB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(pow2x3_kernel<LP, V, TWB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
     if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
-    pow2x3_kernel<LP, V, TWB><<<(unsigned)ntiles, LP, smem, stream>>>(p);
+    pow2x3_kernel<LP, V, TWB, NB><<<(unsigned)ntiles, NB * (LP / P), smem, stream>>>(p);
     return cudaGetLastError();
+}
+
+template <int LP, int NB>
+cudaError_t launch_x3_nb(const PassDesc& p, int variant, int twb, cudaStream_t st)
+{
+    if (twb == TWB_TILE) {
+        if (variant == V_FWD) return launch_x3_one<LP, V_FWD, TWB_TILE, NB>(p, st);
+        if (variant == V_INV) return launch_x3_one<LP, V_INV, TWB_TILE, NB>(p, st);
+    } else if (twb == TWB_LANE) {
+        if (variant == V_FWD) return launch_x3_one<LP, V_FWD, TWB_LANE, NB>(p, st);
+        if (variant == V_INV) return launch_x3_one<LP, V_INV, TWB_LANE, NB>(p, st);
+    }
+    return cudaErrorInvalidValue;
 }
 
 template <int LP>
 cudaError_t launch_x3(const PassDesc& p, int variant, int twb, cudaStream_t st)
 {
-    if (twb == TWB_TILE) {
-        if (variant == V_FWD) return launch_x3_one<LP, V_FWD, TWB_TILE>(p, st);
-        if (variant == V_INV) return launch_x3_one<LP, V_INV, TWB_TILE>(p, st);
-    } else if (twb == TWB_LANE) {
-        if (variant == V_FWD) return launch_x3_one<LP, V_FWD, TWB_LANE>(p, st);
-        if (variant == V_INV) return launch_x3_one<LP, V_INV, TWB_LANE>(p, st);
-    }
+    if (p.nl == 16) return launch_x3_nb<LP, 16>(p, variant, twb, st);
+    if (p.nl == 32) return launch_x3_nb<LP, 32>(p, variant, twb, st);
     return cudaErrorInvalidValue;
 }
 
