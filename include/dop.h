@@ -37,6 +37,16 @@
  *              before anything is enqueued.  No exception crosses the boundary, there is no
  *              global state, and there is NO CPU fallback: without an sm_100 device the
  *              propagate calls fail with DOP_ERR_ARCH / DOP_ERR_CUDA.
+ *
+ * Tuning knobs (environment, read once by dop_plan_create; none changes a result beyond rounding
+ * order, all are exercised by tests/):
+ *   DOP_XDIGITS, DOP_YDIGITS  "a,b[,c]"  force the digit decomposition of an axis (product = length)
+ *   DOP_FORCE_GENERIC         any value  use the generic shared-memory kernel for every pass
+ *   DOP_COL_NB                16|32|64   columns per column-tile bundle of the register-blocked kernels
+ *   DOP_PREFETCH_WAVES        0..64      inter-CTA L2 prefetch distance in waves (0 = off, default 1)
+ *   DOP_SLAB_MB, DOP_SLAB_STREAMS        run multi-pass segments slab by slab on auxiliary streams
+ *                                         (default off)
+ *   DOP_TILE_PTS              256..16384 tile size of the generic kernel
  */
 #ifndef DOP_H_
 #define DOP_H_

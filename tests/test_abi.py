@@ -144,3 +144,20 @@ def test_launch_count_follows_the_slab_schedule(monkeypatch):
     dop.dop_plan_destroy(h)
     # x segments: rows of 16 KiB -> 64 rows per slab -> 16 slabs; y segments: columns of 8 KiB -> 128 -> 16 slabs
     assert n == 13 * 16 + 1
+
+
+@pytest.mark.parametrize("ny,nx,yd,xd,expect", [
+    (65536, 32, "256,256", "32", ["y0 L=256 tile=32x256 col pow2", "y1 L=256 tile=16x256 col pow2"]),
+    (16, 131072, "16", "256,512", ["x0 L=256 tile=16x256 col pow2", "x1 L=512 tile=8x512 row pow2"]),
+    (6144, 128, "384,16", "128", ["y0 L=384 tile=32x384 col pow2", "x0 L=128 tile=32x128 row pow2"]),
+    (64, 8192, "64", "8192", ["x0 L=8192 tile=1x8192 row pow2", "y0 L=64 tile=16x64 col pow2"]),
+])
+def test_plan_routes_digits_to_the_specialised_kernels(ny, nx, yd, xd, expect, monkeypatch):
+    """dop_plan_describe names, per pass, the tile shape and the kernel family the plan chose."""
+    monkeypatch.setenv("DOP_YDIGITS", yd)
+    monkeypatch.setenv("DOP_XDIGITS", xd)
+    h, _ = dop.dop_plan_create(ny, nx, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0)
+    text = dop.dop_plan_describe(h)
+    dop.dop_plan_destroy(h)
+    for e in expect:
+        assert e in text, (e, text)

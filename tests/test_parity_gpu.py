@@ -127,6 +127,46 @@ def test_every_digit_decomposition_gives_the_same_answer(env, monkeypatch):
     assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
 
 
+KERNEL_FAMILIES = [
+    # (ny, nx, DOP_YDIGITS, DOP_XDIGITS): every digit length of every specialised kernel family
+    (256, 1024, "16,16", "16,64"),        # column 16 (tile / H / lane), row 64
+    (1024, 4096, "32,32", "32,128"),      # column 32, row 128
+    (4096, 64, "64,64", "64"),            # column 64 (tile, H), single-digit row 64
+    (16, 16384, "16", "64,256"),          # column 64 (lane), staged row 256
+    (16384, 64, "128,128", "64"),         # column 128 (tile, H)
+    (16, 32768, "16", "128,256"),         # column 128 (lane)
+    (65536, 32, "256,256", "32"),         # column 256 with 32-column bundles (tile), column 256 (H)
+    (16, 131072, "16", "256,512"),        # column 256 (lane), row 512 (runs of 2)
+    (8192, 64, "512,16", "64"),           # column 512 (tile)
+    (8192, 64, "16,512", "64"),           # column 512 (H)
+    (2, 524288, "2", "512,1024"),         # column 512 (lane), row 1024
+    (256, 2048, "16,16", "2048"),         # row 2048
+    (128, 4096, "128", "4096"),           # row 4096
+    (64, 8192, "64", "8192"),             # row 8192 (config 2's)
+    (768, 128, "48,16", "128"),           # 3 x 16
+    (1536, 128, "96,16", "128"),          # 3 x 32
+    (3072, 128, "192,16", "128"),         # 3 x 64
+    (6144, 128, "384,16", "128"),         # 3 x 128 (config 5's)
+    (16, 49152, "16", "16,48,64"),        # 3 x 16 with per-lane boundary twiddles
+]
+
+
+@pytest.mark.parametrize("ny,nx,yd,xd", KERNEL_FAMILIES)
+def test_every_kernel_family_against_the_oracle(ny, nx, yd, xd, monkeypatch):
+    """Forces digit decompositions so that each instantiated digit length of the register-blocked
+    kernels (column tile / H / per-lane variants, staged and unstaged row tiles, 3 x 2^k) runs the
+    fused L2 path and is compared with the oracle."""
+    monkeypatch.setenv("DOP_YDIGITS", yd)
+    monkeypatch.setenv("DOP_XDIGITS", xd)
+    cfg = synth.CONFIGS["C4"].scaled(ny, nx)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I, L, g = run_l2(cfg, h, T)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
 def test_slab_schedule_gives_the_same_answer(monkeypatch):
     """DOP_SLAB_MB: multi-pass segments run slab by slab on auxiliary streams (fork / join on the
     caller's stream); 1 MiB slabs split this grid into 16 column slabs and 16 row slabs."""
