@@ -184,6 +184,32 @@ def test_slab_schedule_gives_the_same_answer(monkeypatch):
     assert abs(L1 - Lr) <= TOL_LOSS * abs(Lr)
 
 
+def test_calls_capture_into_a_cuda_graph():
+    """dop_propagate_fwd / _adj only enqueue kernels on the caller's stream (dop.h "Asynchrony"), so a
+    warmed-up pair captures into a CUDA graph; replays give the bit-identical result."""
+    cfg = synth.CONFIGS["C1"].scaled(256, 512)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, 0.0, 0, DEV)
+    grad = torch.empty_like(h)
+    loss = torch.zeros(1, dtype=torch.float64, device=DEV)
+    plan.fwd(h, T, None, loss)
+    plan.adj(h, None, grad)
+    torch.cuda.synchronize()
+    g0, l0 = grad.clone(), loss.clone()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        plan.fwd(h, T, None, loss)
+        plan.adj(h, None, grad)
+    for _ in range(2):
+        grad.zero_()
+        loss.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(grad, g0) and torch.equal(loss, l0)
+    del graph
+    plan.close()
+
+
 def test_degenerate_inputs():
     """z = 0 (identity on a grid without evanescent bins), flat height (plane wave), negative z."""
     cfg = synth.CONFIGS["C1"].scaled(64, 96)
