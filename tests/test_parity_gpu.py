@@ -262,6 +262,38 @@ def test_repeatable_bitwise():
     assert np.array_equal(a[0], b[0]) and a[1] == b[1] and np.array_equal(a[2], b[2])
 
 
+@pytest.mark.parametrize("ny,nx,yd,xd", [
+    (64, 16384, "64", "64,256"),     # staged row tiles, warp-local exchanges only (256-point rows)
+    (512, 1024, "32,16", "1024"),    # row tiles with one CTA-wide and one warp-local exchange
+    (256, 8192, "16,16", "8192"),    # 8192-point rows (runs of 2 slots, CTA-wide exchanges)
+    (65536, 32, "256,256", "32"),    # 32-column bundles
+    (6144, 128, "384,16", "128"),    # 3 x 128
+])
+def test_repeatable_bitwise_under_load(ny, nx, yd, xd, monkeypatch):
+    """A missing barrier (the row kernels synchronise most exchanges with __syncwarp only) would show
+    as run-to-run differences: the full grid keeps every SM busy with several CTAs, 8 repeats."""
+    monkeypatch.setenv("DOP_YDIGITS", yd)
+    monkeypatch.setenv("DOP_XDIGITS", xd)
+    cfg = synth.CONFIGS["C4"].scaled(ny, nx)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, 0.0,
+                    dop.DOP_WRITE_INTENSITY, DEV)
+    inten = torch.empty((1, ny, nx), dtype=torch.float32, device=DEV)
+    grad = torch.empty_like(h)
+    loss = torch.zeros(1, dtype=torch.float64, device=DEV)
+    ref = None
+    for _ in range(8):
+        plan.fwd(h, T, inten, loss)
+        plan.adj(h, None, grad)
+        torch.cuda.synchronize()
+        cur = (inten.clone(), grad.clone(), loss.clone())
+        if ref is None:
+            ref = cur
+        else:
+            assert all(torch.equal(a, b) for a, b in zip(ref, cur))
+    plan.close()
+
+
 # ------------------------------------------------------------------------------------------------
 # BASELINE.json configurations at full size, in the launch configuration bench.py times
 # ------------------------------------------------------------------------------------------------
