@@ -106,7 +106,7 @@ dop_status ensure_device(dop_plan* p)
 PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b, char* ws)
 {
     PassDesc d{};
-    tile_geometry(p, t.axis, t.digit, &d);
+    pass_geometry(p, t, &d);
     const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
     char* arena = (char*)p->d_arena;
     const size_t npts = (size_t)p->desc.nx * (size_t)p->desc.ny;
@@ -465,7 +465,7 @@ int64_t dop_plan_launch_count(const dop_plan* p)
             size_t j = i + 1;
             while (j < sched.size() && sched[j].axis == sched[i].axis) ++j;
             std::vector<PassDesc> d(j - i);
-            for (size_t k = i; k < j; ++k) tile_geometry(p, sched[k].axis, sched[k].digit, &d[k - i]);
+            for (size_t k = i; k < j; ++k) pass_geometry(p, sched[k], &d[k - i]);
             long long total = 0, per = 0;
             const bool slabbed = slab_layout(p, d, sched[i].axis, &total, &per);
             n += (int64_t)(j - i) * (slabbed ? (total + per - 1) / per : 1);

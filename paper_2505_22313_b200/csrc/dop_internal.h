@@ -99,7 +99,7 @@ struct PassDesc {
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream);
 // register-blocked power-of-two fast path (kernels_pow2.cu)
 bool pow2_supported(long long L, bool col_type);
-int pow2_lines(long long L, bool col_type, bool plain_y = false);
+int pow2_lines(long long L, bool col_type, bool plain = false);
 std::vector<float2> pow2_group_twiddles(long long L);
 cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
                                cudaStream_t stream);
@@ -187,4 +187,5 @@ namespace dop {
 dop_status build_plan(dop_plan* p);
 std::string describe_plan(const dop_plan* p);
 void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d);
+void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d);
 } // namespace dop

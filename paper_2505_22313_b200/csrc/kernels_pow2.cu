@@ -27,15 +27,15 @@ bool pow2_supported(long long L, bool col_type)
     return col_type ? L <= 512 : (L >= 64 && L <= 8192);
 }
 
-// Lines per tile.  Column tiles: the bundle width NB.  `plain_y` = a non-last y digit (plain
-// forward / inverse passes only): measured on B200 (C4, L = 256) 32-column bundles (256-byte
-// segments, 512-thread CTAs) take the plain y passes from 0.67 to 0.75 of the measured copy
-// bandwidth, but cost the register-heavy fused variants 15-30 %, so only those digits get them.
+// Lines per tile.  Column tiles: the bundle width NB.  `plain` = a plain forward / inverse pass or
+// the exp(i Phi) pass: measured on B200, 32-column bundles (256-byte segments) take those from
+// 0.67-0.71 to 0.75-0.83 of the measured copy bandwidth (C4 L = 256, C3 L = 128), but cost the
+// register-heavy fused variants (H, loss) 15-30 %, and 64 columns lose everywhere.
 // DOP_COL_NB = 16 | 32 | 64 overrides for every column tile (clamped to what is instantiated).
-int pow2_lines(long long L, bool col_type, bool plain_y)
+int pow2_lines(long long L, bool col_type, bool plain)
 {
     if (!col_type) return row_lines((int)L);
-    int nb = (plain_y && L >= 256) ? 32 : 16;
+    int nb = (plain && L >= 128) ? 32 : 16;
     if (L % 3 == 0) { // 3 * 2^k digits: 16 or 32 columns
         if (const char* e = std::getenv("DOP_COL_NB")) nb = std::atoi(e) == 32 ? 32 : (std::atoi(e) == 16 ? 16 : nb);
         return nb;

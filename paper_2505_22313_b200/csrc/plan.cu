@@ -139,7 +139,7 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         // column-type unless it is the last x digit
         const bool col_type = !(a == 0 && d.st == 1);
         const long long lines = col_type ? (a == 0 ? d.st : p->desc.nx) : p->desc.ny * (N / d.L);
-        d.fast = !p->force_generic && pow2_supported(d.L, col_type) && lines % pow2_lines(d.L, col_type, a == 1 && d.has_twb) == 0;
+        d.fast = !p->force_generic && pow2_supported(d.L, col_type) && lines % (col_type ? 16 : pow2_lines(d.L, false)) == 0;
         if (d.fast) d.twg = pow2_group_twiddles(d.L);
         if (d.fast && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
             const long long Nj = d.L * d.st;
@@ -254,7 +254,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
         d->n_m = nx / (L * st); d->SM = L * st;
         d->n_o = ny; d->SO = nx;
         d->r_from = 0;
-        d->nl = fast ? pow2_lines(L, true) : (int)std::min<long long>(std::max<long long>(nl_target, 16), st);
+        d->nl = fast ? 16 : (int)std::min<long long>(std::max<long long>(nl_target, 16), st);
     } else { // y digit: lines are adjacent columns, elements st rows apart
         d->col_type = 1;
         d->es = st * nx;
@@ -263,11 +263,31 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
         d->n_o = ny / (L * st); d->SO = L * st * nx;
         d->r_from = 1;
         d->row_o = L * st; d->row_m = 1; d->row_i = st;
-        d->nl = fast ? pow2_lines(L, true, g.has_twb) : (int)std::min<long long>(std::max<long long>(nl_target, 16), nx);
+        d->nl = fast ? 16 : (int)std::min<long long>(std::max<long long>(nl_target, 16), nx);
     }
     d->n_cgroups = (d->NC + d->nl - 1) / d->nl;
     d->smem_bytes = (int)((long long)d->nl * L * (long long)sizeof(float2));
     d->threads = 256;
+}
+
+// Geometry of one scheduled pass: tile_geometry of its digit, then the column bundle width, which
+// is a property of the pass (it does not change where data lives): plain forward / inverse
+// passes (and the exp(i Phi) pass of short digits) take wider bundles (pow2_lines), the register-heavy fused
+// variants stay at 16 columns.
+void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d)
+{
+    tile_geometry(p, t.axis, t.digit, d);
+    const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
+    if (!g.fast || !d->col_type) return;
+    // (the exp(i Phi) pass: measured better at 32 columns for L = 128, worse for L = 256)
+    const bool plain = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.store_op == ST_C64 &&
+                       (t.load_op == LD_C64 || (t.load_op == LD_HEIGHT && g.L <= 128));
+    const int nb = pow2_lines(g.L, true, plain);
+    if (nb != d->nl && d->NC % nb == 0) {
+        d->nl = nb;
+        d->n_cgroups = d->NC / nb;
+        d->smem_bytes = (int)((long long)nb * g.L * (long long)sizeof(float2));
+    }
 }
 
 dop_status build_plan(dop_plan* p)
@@ -334,7 +354,7 @@ std::string describe_plan(const dop_plan* p)
     auto dump = [&](const char* tag, const std::vector<PassTmpl>& v) {
         for (const PassTmpl& t : v) {
             PassDesc g{};
-            tile_geometry(p, t.axis, t.digit, &g);
+            pass_geometry(p, t, &g);
             os << tag << " " << (t.axis == 0 ? "x" : "y") << t.digit << " L=" << g.L << " tile=" << g.nl << "x" << g.L
                << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? " pow2" : " generic") << " ctas=" << g.n_cgroups * g.n_m * g.n_o
                << " smem=" << g.smem_bytes << " B/pt=" << t.bytes_per_point << " [" << t.name << "]\n";
