@@ -152,10 +152,10 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
         const long long threads = d.col_type ? d.L : (long long)d.nl * d.L / 16;
         const long long per_sm = threads > 0 ? (1024 / threads > 0 ? 1024 / threads : 1) : 1;
         d.pf_ahead = (int)(p->pf_waves * 148 * per_sm);
-        // Measured (C2 / C4): a gain on row-type tiles and on y tiles whose
-        // lines span <= 1 GiB; a loss on column tiles with larger spans and on x column tiles.
-        const double span = (double)d.L * (double)d.es * sizeof(float2);
-        if (d.col_type && !(d.r_from == 1 && span <= 1073741824.0)) d.pf_ahead = 0;
+        // Measured (C2 / C3 / C4): a gain on row-type tiles (C3 x passes 0.86 -> 0.75 ms, C2 loss pass
+        // 0.57 -> 0.52 ms); on column tiles a loss, or a wash that over-fetches DRAM by 15-50 %
+        // (ncu) -- with 32-column bundles the C2 y passes run 0.217 ms with it and 0.204 ms without.
+        if (d.col_type) d.pf_ahead = 0;
     }
     d.fx2 = p->d_f2[0];
     d.fy2 = p->d_f2[1];

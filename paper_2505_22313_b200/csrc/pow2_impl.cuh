@@ -264,10 +264,10 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
 
-    // (not compiled into the x column tiles: it never pays there and its registers cost the loss
-    // variant 25%, C4 32 -> 41 ms)
-    if (!COL || TWB != TWB_LANE)
-        prefetch_tile<COL, tile_threads(L, COL, NB), COL ? NB : LINES, (V != V_HEIGHT && V != V_LDOTHER),
+    // (row tiles only: on column tiles it measured as a loss or as a wash that over-fetches DRAM, and
+    // its registers cost the fused variants up to 25 %)
+    if (!COL)
+        prefetch_tile<COL, tile_threads(L, COL, NB), LINES, (V != V_HEIGHT && V != V_LDOTHER),
                       (V == V_HEIGHT || V == V_GRAD), (V == V_LOSS)>(p, 1, L);
 
     // Touch the tables this tile will need after its DFT now, so they are in L1 by then.
@@ -484,8 +484,6 @@ pow2x3_kernel(const __grid_constant__ PassDesc p)
         tws = (unsigned)p.NC;
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
-
-    prefetch_tile<true, NB * (LP / P), NB, true, false, false>(p, 3, 3 * LP);
 
     float2 v[3][P];
     if (DIR > 0) {
