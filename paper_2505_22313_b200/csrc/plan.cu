@@ -280,8 +280,12 @@ void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d)
     const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
     if (!g.fast || !d->col_type) return;
     // (the exp(i Phi) pass: measured better at 32 columns for L = 128, worse for L = 256)
-    const bool plain = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.store_op == ST_C64 &&
-                       (t.load_op == LD_C64 || (t.load_op == LD_HEIGHT && g.L <= 128));
+    // and the gradient / real-plane stores: +5-10 % at 32 columns for L = 128, no change for L = 256)
+    const bool short_digit = g.L <= 128;
+    const bool plain = t.mid_op == MID_NONE && t.fft2_dir == 0 &&
+                       ((t.store_op == ST_C64 && (t.load_op == LD_C64 || (t.load_op == LD_HEIGHT && short_digit))) ||
+                        (t.load_op == LD_C64 && short_digit &&
+                         (t.store_op == ST_GRAD || t.store_op == ST_GRAD_ACC || t.store_op == ST_REAL)));
     const int nb = pow2_lines(g.L, true, plain);
     if (nb != d->nl && d->NC % nb == 0) {
         d->nl = nb;
