@@ -147,6 +147,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.seed_coef = (float)(4.0 / (double)npts);
     d.inv_lam2 = 1.0 / (lambda * lambda);
     d.z = p->desc.z;
+    d.h_fixed = (std::fabs(p->desc.z) / lambda < 524288.0 && std::getenv("DOP_H_FLOAT") == nullptr) ? 1 : 0;
     // prefetch distance in tiles: pf_waves x (148 SMs x resident CTAs of ~1024 threads per SM)
     {
         const long long threads = d.col_type ? d.L : (long long)d.nl * d.L / 16;

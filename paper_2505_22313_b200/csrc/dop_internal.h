@@ -87,6 +87,7 @@ struct PassDesc {
     float scale;          // 1/(ny nx)
     float seed_coef;      // 4/(ny nx)
     double inv_lam2, z;   // H
+    int h_fixed;          // pow2 kernels: |z|/lambda < 2^19, the phase of H may be taken in 32-bit fixed point
     const double* fx2;    // [nx] slot -> fx^2   (fp64, same expression as the definition)
     const double* fy2;    // [ny] slot -> fy^2
     const float* gx;      // [nx] slot -> Gaussian factor

@@ -190,6 +190,59 @@ __device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double f
     return make_float2(0.0f, 0.0f);
 }
 
+// (cos, sin) of a turn fraction given as a 32-bit fixed-point number ph / 2^32: nearest quadrant from
+// the top bits, signed residue (units of 2^-32 turn) rounded to 23 bits and turned into a float with
+// the magic-number trick (no conversion-pipe instruction), then the polynomials of sincos_turn.
+__device__ __forceinline__ void sincos_fixed(unsigned ph, float* sn, float* cs)
+{
+    const unsigned t = ph + 0x20000000u;
+    const int q = (int)(t >> 30);
+    const int ri = (int)(t & 0x3FFFFFFFu) - 0x20000000;                 // [-2^29, 2^29)
+    const float rf = __int_as_float(0x4B400000 + ((ri + 64) >> 7)) - 12582912.0f; // exact, units of 2^-25 turn
+    const float r = rf * 2.98023223876953125e-8f;                      // 2^-25
+    const float r2 = r * r;
+    float sp = fmaf(r2, 42.05869394489765f, -76.70585975306136f);
+    sp = fmaf(sp, r2, 81.60524927607504f);
+    sp = fmaf(sp, r2, -41.34170224039976f);
+    sp = fmaf(sp, r2, 6.283185307179586f);
+    const float s = sp * r;
+    float cp = fmaf(r2, 60.24464137187666f, -85.45681720669373f);
+    cp = fmaf(cp, r2, 64.93939402266829f);
+    cp = fmaf(cp, r2, -19.739208802178716f);
+    const float c = fmaf(cp, r2, 1.0f);
+    const bool odd = (q & 1) != 0;
+    const float co = odd ? s : c, so = odd ? c : s;
+    *cs = __int_as_float(__float_as_int(co) ^ (((q + 1) & 2) << 30));
+    *sn = __int_as_float(__float_as_int(so) ^ ((q & 2) << 30));
+}
+
+// apply_h with the phase taken in fixed point: u = fma(sqrt(a), z 2^32, 1.5 2^52) holds
+// round(turns 2^32) in its low word (valid while |turns| < 2^19; the plan checks |z|/lambda), and the
+// fp32 rsqrt seed goes through bit-level fp64 <-> fp32 conversions.  Per point this replaces three
+// of the four conversion-pipe operations (16 lanes/clk/SM) and three fp64 operations by ~14 integer /
+// fp32 ones.
+__device__ __forceinline__ float2 apply_h_fixed(float2 v, double c_minus_fx2, double fy2, double z32, float scale, bool conj)
+{
+    const double a = c_minus_fx2 - fy2;
+    if (a >= 0.0) {
+        unsigned ph = 0u;
+        if (a > 1e-30) {
+            const int hi = __double2hiint(a), lo = __double2loint(a);
+            const float af = __int_as_float(((hi - 0x38000000) << 3) | (int)((unsigned)lo >> 29)); // truncated (float)a
+            const int yb = __float_as_int(rsqrtf(af));
+            const double y = __hiloint2double((yb >> 3) + 0x38000000, yb << 29);                    // exact (double)y
+            double s = a * y;
+            s = fma(fma(-s, s, a), 0.5 * y, s);
+            ph = (unsigned)__double2loint(fma(s, z32, 6755399441055744.0));
+        }
+        float sn, cs;
+        sincos_fixed(ph, &sn, &cs);
+        const float2 h = make_float2(cs * scale, (conj ? -sn : sn) * scale);
+        return fx::cmul(v, h);
+    }
+    return make_float2(0.0f, 0.0f);
+}
+
 // ---- the tile-pass kernel -------------------------------------------------------------------
 template <int L, bool COL, int V, int TWB, int NB>
 __global__ void __launch_bounds__(tile_threads(L, COL, NB), min_blocks(L, COL, V, NB))
@@ -349,8 +402,14 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         const double* __restrict__ fyp = p.fy2 + o * p.row_o + m * p.row_m + tt * RL;
         const double cfx = p.inv_lam2 - __ldg(p.fx2 + line);
         const bool cj = p.mid_op == MID_HCONJ;
+        if (p.h_fixed) {
+            const double z32 = p.z * 4294967296.0;
 #pragma unroll
-        for (int i = 0; i < P; ++i) v[i] = apply_h(v[i], cfx, __ldg(fyp + DOP_KL(i)), p.z, p.scale, cj);
+            for (int i = 0; i < P; ++i) v[i] = apply_h_fixed(v[i], cfx, __ldg(fyp + DOP_KL(i)), z32, p.scale, cj);
+        } else {
+#pragma unroll
+            for (int i = 0; i < P; ++i) v[i] = apply_h(v[i], cfx, __ldg(fyp + DOP_KL(i)), p.z, p.scale, cj);
+        }
     } else if (V == V_GAUSS) {
         const float* __restrict__ gyp = p.gy + o * p.row_o + m * p.row_m + tt * RL;
         const float gxs = __ldg(p.gx + line) * p.scale;

@@ -184,6 +184,23 @@ def test_slab_schedule_gives_the_same_answer(monkeypatch):
     assert abs(L1 - Lr) <= TOL_LOSS * abs(Lr)
 
 
+@pytest.mark.parametrize("z,env", [(2e-3, {"DOP_H_FLOAT": "1"}), (0.4, {}), (-0.4, {}), (0.28, {})])
+def test_both_phase_paths_of_H(z, env, monkeypatch):
+    """H's phase is taken in 32-bit fixed point while |z|/lambda < 2^19 turns and through the fp32
+    fraction otherwise (or with DOP_H_FLOAT): both against the oracle, on both sides of the switch
+    (0.28 m / 550 nm = 509 091 turns < 2^19 = 524 288 <= 0.4 m / 550 nm)."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    import dataclasses
+    cfg = dataclasses.replace(synth.CONFIGS["C4"].scaled(512, 256), z=z)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I, L, g = run_l2(cfg, h, T)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
 def test_calls_capture_into_a_cuda_graph():
     """dop_propagate_fwd / _adj only enqueue kernels on the caller's stream (dop.h "Asynchrony"), so a
     warmed-up pair captures into a CUDA graph; replays give the bit-identical result."""
