@@ -46,6 +46,8 @@
  *   DOP_PREFETCH_WAVES        0..64      inter-CTA L2 prefetch distance in waves (0 = off, default 1)
  *   DOP_SLAB_MB, DOP_SLAB_STREAMS        run multi-pass segments slab by slab on auxiliary streams
  *                                         (default off)
+ *   DOP_H_FLOAT               any value  take the phase of H through an fp32 fraction even when the
+ *                                         fixed-point path applies
  *   DOP_TILE_PTS              256..16384 tile size of the generic kernel
  */
 #ifndef DOP_H_

@@ -147,7 +147,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.seed_coef = (float)(4.0 / (double)npts);
     d.inv_lam2 = 1.0 / (lambda * lambda);
     d.z = p->desc.z;
-    d.h_fixed = (std::fabs(p->desc.z) / lambda < 524288.0 && std::getenv("DOP_H_FLOAT") == nullptr) ? 1 : 0;
+    d.h_fixed = (std::fabs(p->desc.z) / lambda < 524288.0 && !p->h_float) ? 1 : 0;
     // prefetch distance in tiles: pf_waves x (148 SMs x resident CTAs of ~1024 threads per SM)
     {
         const long long threads = d.col_type ? d.L : (long long)d.nl * d.L / 16;
@@ -245,9 +245,7 @@ dop_status run_segment(dop_plan* p, const std::vector<PassTmpl>& sched, size_t b
     }
     // lazily create the auxiliary streams (DOP_SLAB_STREAMS, default 2)
     if (p->n_aux == 0) {
-        int ns = 2;
-        if (const char* e = std::getenv("DOP_SLAB_STREAMS")) ns = std::atoi(e);
-        ns = ns < 1 ? 1 : (ns > 4 ? 4 : ns);
+        const int ns = p->slab_streams;
         if (cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess) return DOP_ERR_CUDA;
         for (int k = 0; k < ns; ++k) {
             if (cudaStreamCreateWithFlags(&p->aux[k], cudaStreamNonBlocking) != cudaSuccess) return DOP_ERR_CUDA;

@@ -100,7 +100,7 @@ struct PassDesc {
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream);
 // register-blocked power-of-two fast path (kernels_pow2.cu)
 bool pow2_supported(long long L, bool col_type);
-int pow2_lines(long long L, bool col_type, bool plain = false);
+int pow2_lines(long long L, bool col_type, bool plain = false, int nb_override = 0);
 std::vector<float2> pow2_group_twiddles(long long L);
 cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
                                cudaStream_t stream);
@@ -154,6 +154,9 @@ struct dop_plan {
     std::vector<long long> wl_len;
     std::vector<size_t> wl_off;
     int tile_pts = 4096;
+    int col_nb = 0;             // DOP_COL_NB override of the column bundle width (0 = per-pass default)
+    bool h_float = false;       // DOP_H_FLOAT: never take H's phase in fixed point
+    int slab_streams = 2;       // DOP_SLAB_STREAMS
     int pf_waves = 1;           // L2 prefetch distance of the pow2 kernels, in waves of resident CTAs (0 = off)
     long long slab_bytes = 0;   // L2 slab size for multi-pass segments (0 = whole-array launches)
     bool force_generic = false; // DOP_FORCE_GENERIC at plan creation: generic kernel for every pass

@@ -31,19 +31,14 @@ bool pow2_supported(long long L, bool col_type)
 // the exp(i Phi) pass: measured on B200, 32-column bundles (256-byte segments) take those from
 // 0.67-0.71 to 0.75-0.83 of the measured copy bandwidth (C4 L = 256, C3 L = 128), but cost the
 // register-heavy fused variants (H, loss) 15-30 %, and 64 columns lose everywhere.
-// DOP_COL_NB = 16 | 32 | 64 overrides for every column tile (clamped to what is instantiated).
-int pow2_lines(long long L, bool col_type, bool plain)
+// nb_override (DOP_COL_NB = 16 | 32 | 64, read at plan creation) applies to every column tile, clamped
+// to what is instantiated.
+int pow2_lines(long long L, bool col_type, bool plain, int nb_override)
 {
     if (!col_type) return row_lines((int)L);
     int nb = (plain && L >= 128) ? 32 : 16;
-    if (L % 3 == 0) { // 3 * 2^k digits: 16 or 32 columns
-        if (const char* e = std::getenv("DOP_COL_NB")) nb = std::atoi(e) == 32 ? 32 : (std::atoi(e) == 16 ? 16 : nb);
-        return nb;
-    }
-    if (const char* e = std::getenv("DOP_COL_NB")) {
-        const int v = std::atoi(e);
-        if (v == 16 || v == 32 || v == 64) nb = v;
-    }
+    if (nb_override == 16 || nb_override == 32 || nb_override == 64) nb = nb_override;
+    if (L % 3 == 0) return nb > 32 ? 32 : nb; // 3 * 2^k digits: 16 or 32 columns
     const int mx = max_col_nb((int)L);
     return nb < mx ? nb : mx;
 }

@@ -286,7 +286,7 @@ void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d)
                        ((t.store_op == ST_C64 && (t.load_op == LD_C64 || (t.load_op == LD_HEIGHT && short_digit))) ||
                         (t.load_op == LD_C64 && short_digit &&
                          (t.store_op == ST_GRAD || t.store_op == ST_GRAD_ACC || t.store_op == ST_REAL)));
-    const int nb = pow2_lines(g.L, true, plain);
+    const int nb = pow2_lines(g.L, true, plain, p->col_nb);
     if (nb != d->nl && d->NC % nb == 0) {
         d->nl = nb;
         d->n_cgroups = d->NC / nb;
@@ -302,6 +302,12 @@ dop_status build_plan(dop_plan* p)
     if (const char* e = std::getenv("DOP_TILE_PTS")) {
         int v = std::atoi(e);
         if (v >= 256 && v <= 16384) p->tile_pts = v;
+    }
+    if (const char* e = std::getenv("DOP_COL_NB")) p->col_nb = std::atoi(e);
+    p->h_float = std::getenv("DOP_H_FLOAT") != nullptr;
+    if (const char* e = std::getenv("DOP_SLAB_STREAMS")) {
+        int v = std::atoi(e);
+        p->slab_streams = v < 1 ? 1 : (v > 4 ? 4 : v);
     }
     if (const char* e = std::getenv("DOP_PREFETCH_WAVES")) {
         int v = std::atoi(e);
