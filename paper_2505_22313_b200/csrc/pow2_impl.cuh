@@ -128,7 +128,7 @@ __device__ __forceinline__ void field_st(float2* p, float2 v)
     else *p = v;
 }
 
-// (cos 2 pi f, sin 2 pi f) for |f| <= 1/2 turn: quadrant q = round(4f) by the magic-number trick
+// (cos 2 pi f, sin 2 pi f) for |f| < 2^20 turns: quadrant q = round(4f) mod 4 by the magic-number trick
 // (no F2I / FRND), residue |r| <= 1/8 turn, Taylor polynomials in r^2 (truncation 2e-9 / 2.4e-8),
 // then the quadrant rotation by selects and sign flips.  ~23 instructions against ~30 for the
 // library sincospif, which also has to handle arbitrary arguments.
@@ -158,13 +158,9 @@ __device__ __forceinline__ void sincos_turn(float f, float* sn, float* cs)
     *cs = __int_as_float(__float_as_int(co) ^ (((q + 1) & 2) << 30));
     *sn = __int_as_float(__float_as_int(so) ^ ((q & 2) << 30));
 }
-// the same for any moderate argument in turns (|ph| < 2^21): reduce to the nearest integer first
-__device__ __forceinline__ void sincos_turns(float ph, float* sn, float* cs)
-{
-    const float MAGIC = 12582912.0f;
-    const float n = (ph + MAGIC) - MAGIC; // round to nearest integer
-    sincos_turn(ph - n, sn, cs);
-}
+// Any moderate argument in turns (|ph| < 2^20) needs no separate integer reduction: round(4 ph) mod 4
+// is the quadrant whatever the integer part, and ph - round(4 ph)/4 is exact (Sterbenz).
+__device__ __forceinline__ void sincos_turns(float ph, float* sn, float* cs) { sincos_turn(ph, sn, cs); }
 
 // F4 / A3: v *= H (or conj H) / N; evanescent bins (a < 0) zeroed.  a and the phase z sqrt(a)
 // are fp64; sqrt = fp32 rsqrt seed + one fp64 Newton step.
