@@ -38,17 +38,9 @@
  *              global state, and there is NO CPU fallback: without an sm_100 device the
  *              propagate calls fail with DOP_ERR_ARCH / DOP_ERR_CUDA.
  *
- * Tuning knobs (environment, read once by dop_plan_create; none changes a result beyond rounding
- * order, all are exercised by tests/):
- *   DOP_XDIGITS, DOP_YDIGITS  "a,b[,c]"  force the digit decomposition of an axis (product = length)
- *   DOP_FORCE_GENERIC         any value  use the generic shared-memory kernel for every pass
- *   DOP_COL_NB                16|32|64   columns per column-tile bundle of the register-blocked kernels
- *   DOP_PREFETCH_WAVES        0..64      inter-CTA L2 prefetch distance in waves (0 = off, default 1)
- *   DOP_SLAB_MB, DOP_SLAB_STREAMS        run multi-pass segments slab by slab on auxiliary streams
- *                                         (default off)
- *   DOP_H_FLOAT               any value  take the phase of H through an fp32 fraction even when the
- *                                         fixed-point path applies
- *   DOP_TILE_PTS              256..16384 tile size of the generic kernel
+ * Tuning (dop_tuning, passed explicitly through dop_plan_desc.tuning; NULL = defaults).  The library
+ * reads NO environment variable and keeps no global state.  None of the fields changes a result
+ * beyond rounding order; tests/ exercises every one of them.
  */
 #ifndef DOP_H_
 #define DOP_H_
@@ -81,6 +73,25 @@ typedef enum {
 /* flags */
 #define DOP_WRITE_INTENSITY 0x1u /* DOP_LOSS_L2 only: also write I to d_intensity                */
 
+/* Optional tuning of the pass schedule (measurement and test aid).  Zero-initialise, then set fields. */
+typedef struct {
+    int32_t n_xdigits;      /* > 0: force the digit decomposition of the x axis (product must be nx,   */
+    int64_t xdigits[4];     /*      every digit within the kernels' limits, else UNSUPPORTED_SIZE)     */
+    int32_t n_ydigits;      /* the same for the y axis                                                  */
+    int64_t ydigits[4];
+    int32_t force_generic;  /* != 0: generic shared-memory kernel for every pass                        */
+    int32_t col_nb;         /* 16 | 32 | 64: columns per column-tile bundle (0 = per-pass default)      */
+    int32_t prefetch_waves; /* 1..64: inter-CTA L2 prefetch distance in waves; -1 = off; 0 = default 1  */
+    int32_t slab_mb;        /* > 0: run multi-pass segments slab by slab    */
+    int32_t slab_streams;   /* 1..4 auxiliary streams of the slab schedule (0 = default 2)              */
+    int32_t h_float;        /* != 0: take the phase of H through an fp32 fraction, never fixed point    */
+    int32_t tile_pts;       /* 256..16384: tile size of the generic kernel (0 = default 4096)           */
+    int32_t no_cluster;     /* != 0: never use the thread-block-cluster row kernels (long x axes then   */
+                            /*       run as two digit passes)                                           */
+    int32_t no_mirror;      /* != 0: do not pair mirrored ky tiles in the (x) H pass                    */
+    int32_t reserved[7];    /* must be 0                                                                */
+} dop_tuning;
+
 typedef struct {
     int64_t ny, nx;            /* rows, columns; x contiguous; each 2^a 3^b, >= 2               */
     double pitch;              /* metres, same in x and y                                        */
@@ -91,6 +102,7 @@ typedef struct {
     dop_loss_mode loss;
     double prefilter_sigma_px; /* 0 = off; > 0 = Gaussian spectral pre-filter on h (config 3)    */
     uint32_t flags;            /* DOP_WRITE_INTENSITY                                            */
+    const dop_tuning* tuning;  /* HOST, copied; NULL = defaults                                  */
 } dop_plan_desc;
 
 /*

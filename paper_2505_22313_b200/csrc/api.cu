@@ -158,6 +158,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
         // (ncu) -- with 32-column bundles the C2 y passes run 0.217 ms with it and 0.204 ms without.
         if (d.col_type) d.pf_ahead = 0;
     }
+    d.device = p->device;
     d.fx2 = p->d_f2[0];
     d.fy2 = p->d_f2[1];
     d.gx = p->d_g[0];
@@ -236,7 +237,9 @@ dop_status run_segment(dop_plan* p, const std::vector<PassTmpl>& sched, size_t b
     const bool slabbed = slab_layout(p, d, axis, &total, &per);
     if (!slabbed) { // whole-array launches, one profiling slot per launch
         for (size_t i = b; i < e; ++i) {
-            long long slot = prof_begin(p, pass_label(tag, sched[i]), sched[i].bytes_per_point, st);
+            // (the dL/dh accumulate of every wavelength after the first re-reads grad: +4 B/point)
+            const double bpp = sched[i].bytes_per_point + ((lam > 0 && sched[i].store_op == ST_GRAD) ? 4.0 : 0.0);
+            long long slot = prof_begin(p, pass_label(tag, sched[i]), bpp, st);
             cudaError_t er = launch_tile_pass(d[i - b], st);
             prof_end(p, slot, st);
             if (er != cudaSuccess) return DOP_ERR_CUDA;
@@ -333,6 +336,8 @@ dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* works
     p->n_refr.assign(d->n_refr, d->n_refr + d->n_lambda);
     p->desc.lambda = p->lambda.data();
     p->desc.n_refr = p->n_refr.data();
+    if (d->tuning != nullptr) p->tune = *d->tuning;
+    p->desc.tuning = nullptr;
     dop_status s;
     try {
         s = build_plan(p);

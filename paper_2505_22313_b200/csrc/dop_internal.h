@@ -95,6 +95,7 @@ struct PassDesc {
     long long row_o, row_m, row_i; // y slot of element i: o*row_o + m*row_m + i*row_i
     int smem_bytes;
     int threads;
+    int device;           // the plan's device (function attributes are set once per device)
 };
 
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream);
@@ -148,6 +149,7 @@ struct PassTmpl {
 
 struct dop_plan {
     dop_plan_desc desc;
+    dop_tuning tune{};          // copy of desc.tuning (zeros = defaults)
     std::vector<double> lambda, n_refr;
     dop::Axis ax[2]; // 0 = x, 1 = y
     std::vector<std::vector<float2>> wl_tables; // distinct W_L tables

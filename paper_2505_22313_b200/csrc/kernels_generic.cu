@@ -7,6 +7,8 @@
 // Math (Eq. 1-4; PAPER.md:200 row-column 2-D FFT):
 //   forward digit pass : v <- DFT_L(v) along the line, then v *= T_j      (T_j boundary twiddle)
 //   inverse digit pass : v *= conj(T_j), then v <- L * IDFT_L(v)          (1/N folded into H)
+#include <atomic>
+
 #include "dop_internal.h"
 
 namespace dop {
@@ -251,16 +253,20 @@ cudaError_t launch_tile_pass_generic(const PassDesc& p, cudaStream_t stream)
 {
     const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
     if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
-    cudaError_t e;
-    if (p.col_type) {
-        e = cudaFuncSetAttribute(tile_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, p.smem_bytes);
+    // the > 48 KiB dynamic shared-memory opt-in is per device function AND per device: once each
+    static std::atomic<unsigned long long> attr_mask{0};
+    const unsigned long long bit = (p.device >= 0 && p.device < 64) ? 1ull << p.device : 0ull;
+    if (bit == 0 || !(attr_mask.load(std::memory_order_acquire) & bit)) {
+        const int max_smem = 200 * 1024;
+        cudaError_t e = cudaFuncSetAttribute(tile_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(tile_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
         if (e != cudaSuccess) return e;
-        tile_pass_kernel<true><<<(unsigned)ntiles, p.threads, p.smem_bytes, stream>>>(p);
-    } else {
-        e = cudaFuncSetAttribute(tile_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, p.smem_bytes);
-        if (e != cudaSuccess) return e;
-        tile_pass_kernel<false><<<(unsigned)ntiles, p.threads, p.smem_bytes, stream>>>(p);
+        if (bit != 0) attr_mask.fetch_or(bit, std::memory_order_release);
     }
+    if (p.smem_bytes > 200 * 1024) return cudaErrorInvalidConfiguration;
+    if (p.col_type) tile_pass_kernel<true><<<(unsigned)ntiles, p.threads, p.smem_bytes, stream>>>(p);
+    else tile_pass_kernel<false><<<(unsigned)ntiles, p.threads, p.smem_bytes, stream>>>(p);
     return cudaGetLastError();
 }
 

@@ -79,7 +79,7 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
         if (p.tw_b2 == nullptr || !col) return cudaSuccess;
         twb = p.r_from == 1 ? TWB_TILE : TWB_LANE;
     }
-    cudaError_t e = cudaErrorInvalidValue;
+    cudaError_t e = kNotInstantiated;
     if (p.L % 3 == 0) {
         switch (p.L / 3) {
         case 16: e = launch_x3<16>(p, v, twb, stream); break;
@@ -108,7 +108,7 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
         case 8192: e = launch_L<8192, false>(p, v, twb, stream); break;
         }
     }
-    if (e == cudaErrorInvalidValue) return cudaSuccess; // combination not instantiated: generic kernel
+    if (e == kNotInstantiated) return cudaSuccess; // combination not instantiated: generic kernel
     *handled = true;
     return e;
 }

@@ -3,7 +3,6 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <sstream>
 
@@ -61,23 +60,22 @@ static std::vector<float2> twiddle_table(long long n)
 }
 
 // Split N into the fewest digits with every digit <= lmax_first (all but the last) and the last
-// <= lmax_last, as balanced as possible.  env_name (if set, e.g. "256,256") overrides.
-static bool split_digits(long long N, long long lmax_first, long long lmax_last, const char* env_name,
-                         std::vector<long long>* out)
+// <= lmax_last, as balanced as possible.  A forced decomposition (dop_tuning) overrides; it must
+// multiply to N and respect the same limits.
+static bool split_digits(long long N, long long lmax_first, long long lmax_last, int n_forced,
+                         const int64_t* forced, std::vector<long long>* out)
 {
     out->clear();
-    if (const char* e = env_name ? std::getenv(env_name) : nullptr) {
-        std::vector<long long> v;
+    if (n_forced > 0) {
+        if (n_forced > 4) return false;
         long long prod = 1;
-        std::stringstream ss(e);
-        std::string tok;
-        while (std::getline(ss, tok, ',')) {
-            long long x = std::atoll(tok.c_str());
-            if (x < 2) { v.clear(); break; }
-            v.push_back(x);
+        for (int i = 0; i < n_forced; ++i) {
+            const long long x = forced[i];
+            if (x < 2 || x > (i + 1 < n_forced ? lmax_first : lmax_last)) return false;
+            out->push_back(x);
             prod *= x;
         }
-        if (!v.empty() && prod == N) { *out = v; return true; }
+        return prod == N;
     }
     if (N <= lmax_last) { out->push_back(N); return true; }
     // divisors of N
@@ -298,39 +296,40 @@ dop_status build_plan(dop_plan* p)
 {
     const dop_plan_desc& d = p->desc;
     if (!is_23_smooth(d.nx) || !is_23_smooth(d.ny)) return DOP_ERR_UNSUPPORTED_SIZE;
-    p->force_generic = std::getenv("DOP_FORCE_GENERIC") != nullptr;
-    if (const char* e = std::getenv("DOP_TILE_PTS")) {
-        int v = std::atoi(e);
-        if (v >= 256 && v <= 16384) p->tile_pts = v;
+    const dop_tuning& tu = p->tune;
+    p->force_generic = tu.force_generic != 0;
+    if (tu.tile_pts != 0) {
+        if (tu.tile_pts < 256 || tu.tile_pts > 16384) return DOP_ERR_INVALID_ARG;
+        p->tile_pts = tu.tile_pts;
     }
-    if (const char* e = std::getenv("DOP_COL_NB")) p->col_nb = std::atoi(e);
-    p->h_float = std::getenv("DOP_H_FLOAT") != nullptr;
-    if (const char* e = std::getenv("DOP_SLAB_STREAMS")) {
-        int v = std::atoi(e);
-        p->slab_streams = v < 1 ? 1 : (v > 4 ? 4 : v);
-    }
-    if (const char* e = std::getenv("DOP_PREFETCH_WAVES")) {
-        int v = std::atoi(e);
-        if (v >= 0 && v <= 64) p->pf_waves = v;
-    }
+    if (tu.col_nb != 0 && tu.col_nb != 16 && tu.col_nb != 32 && tu.col_nb != 64) return DOP_ERR_INVALID_ARG;
+    p->col_nb = tu.col_nb;
+    p->h_float = tu.h_float != 0;
+    if (tu.slab_streams < 0 || tu.slab_streams > 4) return DOP_ERR_INVALID_ARG;
+    p->slab_streams = tu.slab_streams == 0 ? 2 : tu.slab_streams;
+    if (tu.prefetch_waves < -1 || tu.prefetch_waves > 64) return DOP_ERR_INVALID_ARG;
+    p->pf_waves = tu.prefetch_waves == 0 ? 1 : (tu.prefetch_waves < 0 ? 0 : tu.prefetch_waves);
     // Multi-pass segments can run slab by slab so that the passes after the first hit L2.  Off by
     // default: measured slower than whole-array launches on B200.
-    p->slab_bytes = 0;
-    if (const char* e = std::getenv("DOP_SLAB_MB")) {
-        int v = std::atoi(e);
-        if (v >= 0 && v <= 4096) p->slab_bytes = (long long)v << 20;
-    }
+    if (tu.slab_mb < 0 || tu.slab_mb > 4096) return DOP_ERR_INVALID_ARG;
+    p->slab_bytes = (long long)tu.slab_mb << 20;
+    for (int i = 0; i < 7; ++i)
+        if (tu.reserved[i] != 0) return DOP_ERR_INVALID_ARG;
     // generic kernel limits: a row-type line <= 8192 points (64 KiB), a column-type digit
     // <= 512 points (x 16 adjacent lines = 64 KiB)
     std::vector<long long> lx, ly;
-    if (!split_digits(d.nx, 512, 8192, "DOP_XDIGITS", &lx)) return DOP_ERR_UNSUPPORTED_SIZE;
-    if (!split_digits(d.ny, 512, 512, "DOP_YDIGITS", &ly)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (!split_digits(d.nx, 512, 8192, tu.n_xdigits, tu.xdigits, &lx)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (!split_digits(d.ny, 512, 512, tu.n_ydigits, tu.ydigits, &ly)) return DOP_ERR_UNSUPPORTED_SIZE;
     if (!build_axis(p, 0, d.nx, lx) || !build_axis(p, 1, d.ny, ly)) return DOP_ERR_UNSUPPORTED_SIZE;
     build_schedule(p);
-    // the MID_LOSS pass is x digit 0
-    PassDesc g{};
-    tile_geometry(p, 0, 0, &g);
-    p->loss_tiles = g.n_cgroups * g.n_m * g.n_o;
+    // CTAs of the MID_LOSS pass, in the geometry it is launched with (one loss partial per CTA)
+    p->loss_tiles = 0;
+    for (const PassTmpl& t : p->fwd)
+        if (t.mid_op == MID_LOSS) {
+            PassDesc g{};
+            pass_geometry(p, t, &g);
+            p->loss_tiles = g.n_cgroups * g.n_m * g.n_o;
+        }
     // workspace: [n_lambda fields][h_eff plane][loss partials]
     const size_t npts = (size_t)d.nx * (size_t)d.ny;
     auto align256 = [](size_t x) { return (x + 255) & ~(size_t)255; };
@@ -350,7 +349,7 @@ std::string describe_plan(const dop_plan* p)
     const dop_plan_desc& d = p->desc;
     os << "grid ny=" << d.ny << " nx=" << d.nx << " n_lambda=" << d.n_lambda
        << " loss=" << (d.loss == DOP_LOSS_L2 ? "L2" : "none") << " prefilter_sigma_px=" << d.prefilter_sigma_px
-       << " workspace_bytes=" << p->ws_bytes << "\n";
+       << " workspace_bytes=" << p->ws_bytes << " loss_tiles=" << p->loss_tiles << "\n";
     for (int a = 0; a < 2; ++a) {
         os << (a == 0 ? "x" : "y") << "-digits:";
         for (const Digit& g : p->ax[a].dig) {
@@ -376,6 +375,8 @@ std::string describe_plan(const dop_plan* p)
     dump("adj", p->adj);
     dump("pre-adj", p->pre);
     os << "algorithmic_bytes_per_point=" << total << "\n";
+    if (d.n_lambda > 1)
+        os << "(per wavelength; every wavelength after the first re-reads dL/dh to accumulate: +4 B/point on its last pass)\n";
     return os.str();
 }
 

@@ -10,10 +10,32 @@
 // boundary-twiddle mode), so the emitted code has no per-element branches and its addresses are
 // base + compile-time multiples of one stride.
 #pragma once
+#include <atomic>
+
 #include "dop_internal.h"
 #include "fft_regs.cuh"
 
 namespace dop {
+
+// "this (digit, variant, twiddle mode, bundle) combination is not instantiated": the dispatcher then
+// falls back to the generic kernel.  Deliberately not a value of the CUDA error enum, so that a real
+// launch failure can never be mistaken for it.
+constexpr cudaError_t kNotInstantiated = (cudaError_t)0x7fff0001;
+
+// cudaFuncSetAttribute acts on the CURRENT device only: remember, per kernel instantiation, on which
+// devices it has been applied (a second plan on another GPU of the same process must set it again).
+struct AttrOnce {
+    std::atomic<unsigned long long> mask{0};
+    template <class F>
+    cudaError_t ensure(int dev, F&& set)
+    {
+        const unsigned long long bit = (dev >= 0 && dev < 64) ? 1ull << dev : 0ull;
+        if (bit != 0 && (mask.load(std::memory_order_acquire) & bit)) return cudaSuccess;
+        cudaError_t e = set();
+        if (e == cudaSuccess && bit != 0) mask.fetch_or(bit, std::memory_order_release);
+        return e;
+    }
+};
 
 using fx::P;
 
@@ -428,7 +450,11 @@ pow2_kernel(const __grid_constant__ PassDesc p)
             if (p.write_intensity) p.plane_out[off] = I;
         }
         // deterministic CTA reduction: warp shuffle tree, then thread 0 in warp order
-        for (int d = 16; d > 0; d >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, d);
+        constexpr int NT = tile_threads(L, COL, NB);
+        constexpr int SW = NT < 32 ? NT : 32;                         // a 16-thread CTA (L = 16, 16 columns) is half a warp
+        constexpr unsigned SMASK = NT < 32 ? (1u << SW) - 1u : 0xffffffffu;
+#pragma unroll
+        for (int d = SW / 2; d > 0; d >>= 1) acc += __shfl_down_sync(SMASK, acc, d, SW);
         if ((tid & 31) == 0) red[tid >> 5] = acc;
         __syncthreads();
         if (tid == 0) {
@@ -603,12 +629,11 @@ template <int LP, int V, int TWB, int NB>
 static cudaError_t launch_x3_one(const PassDesc& p, cudaStream_t stream)
 {
     constexpr int smem = fx::Tile<LP, true, NB>::LINE_ELEMS * (int)sizeof(float2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(pow2x3_kernel<LP, V, TWB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    static AttrOnce once;
+    cudaError_t e = once.ensure(p.device, [] {
+        return cudaFuncSetAttribute(pow2x3_kernel<LP, V, TWB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    });
+    if (e != cudaSuccess) return e;
     const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
     if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
     pow2x3_kernel<LP, V, TWB, NB><<<(unsigned)ntiles, NB * (LP / P), smem, stream>>>(p);
@@ -625,7 +650,7 @@ cudaError_t launch_x3_nb(const PassDesc& p, int variant, int twb, cudaStream_t s
         if (variant == V_FWD) return launch_x3_one<LP, V_FWD, TWB_LANE, NB>(p, st);
         if (variant == V_INV) return launch_x3_one<LP, V_INV, TWB_LANE, NB>(p, st);
     }
-    return cudaErrorInvalidValue;
+    return kNotInstantiated;
 }
 
 template <int LP>
@@ -633,7 +658,7 @@ cudaError_t launch_x3(const PassDesc& p, int variant, int twb, cudaStream_t st)
 {
     if (p.nl == 16) return launch_x3_nb<LP, 16>(p, variant, twb, st);
     if (p.nl == 32) return launch_x3_nb<LP, 32>(p, variant, twb, st);
-    return cudaErrorInvalidValue;
+    return kNotInstantiated;
 }
 
 // ---- host side -------------------------------------------------------------------------------
@@ -643,22 +668,21 @@ static cudaError_t launch_one(const PassDesc& p, cudaStream_t stream)
     using TL = fx::Tile<L, COL, NB>;
     constexpr int threads = tile_threads(L, COL, NB);
     constexpr int smem = (COL ? 1 : row_lines(L)) * TL::LINE_ELEMS * (int)sizeof(float2);
-    static bool attr_done = false; // per instantiation; the attribute is per device function
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB, NB>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                 cudaSharedmemCarveoutMaxShared);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    static AttrOnce once; // per instantiation and device
+    cudaError_t e = once.ensure(p.device, [] {
+        cudaError_t a = cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (a != cudaSuccess) return a;
+        return cudaFuncSetAttribute(pow2_kernel<L, COL, V, TWB, NB>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                    cudaSharedmemCarveoutMaxShared);
+    });
+    if (e != cudaSuccess) return e;
     const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
     if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
     pow2_kernel<L, COL, V, TWB, NB><<<(unsigned)ntiles, threads, smem, stream>>>(p);
     return cudaGetLastError();
 }
 
-// All variants of one (L, tile type).  Returns cudaErrorInvalidValue for a combination that is
+// All variants of one (L, tile type).  Returns kNotInstantiated for a combination that is
 // never scheduled (the dispatcher then falls back to the generic kernel).
 // widest column bundle instantiated for a digit length: 64 columns up to L = 128, 32 up to 256
 __host__ __device__ constexpr int max_col_nb(int L) { return L <= 128 ? 64 : (L <= 256 ? 32 : 16); }
@@ -685,10 +709,10 @@ cudaError_t launch_col(const PassDesc& p, int variant, int twb, cudaStream_t st)
             }
         }
     }
-    return cudaErrorInvalidValue;
+    return kNotInstantiated;
 }
 
-// All variants of one (L, tile type).  Returns cudaErrorInvalidValue for a combination that is
+// All variants of one (L, tile type).  Returns kNotInstantiated for a combination that is
 // never scheduled (the dispatcher then falls back to the generic kernel).
 template <int L, bool COL>
 cudaError_t launch_L(const PassDesc& p, int variant, int twb, cudaStream_t st)
@@ -710,7 +734,7 @@ cudaError_t launch_L(const PassDesc& p, int variant, int twb, cudaStream_t st)
             }
         }
     }
-    return cudaErrorInvalidValue;
+    return kNotInstantiated;
 }
 
 } // namespace dop

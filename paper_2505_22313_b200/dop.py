@@ -25,12 +25,38 @@ DOP_LOSS_L2 = 1
 DOP_WRITE_INTENSITY = 0x1
 
 
+class dop_tuning(C.Structure):
+    _fields_ = [
+        ("n_xdigits", C.c_int32), ("xdigits", C.c_int64 * 4), ("n_ydigits", C.c_int32), ("ydigits", C.c_int64 * 4),
+        ("force_generic", C.c_int32), ("col_nb", C.c_int32), ("prefetch_waves", C.c_int32), ("slab_mb", C.c_int32),
+        ("slab_streams", C.c_int32), ("h_float", C.c_int32), ("tile_pts", C.c_int32), ("no_cluster", C.c_int32),
+        ("no_mirror", C.c_int32), ("reserved", C.c_int32 * 7),
+    ]
+
+
 class dop_plan_desc(C.Structure):
     _fields_ = [
         ("ny", C.c_int64), ("nx", C.c_int64), ("pitch", C.c_double), ("n_lambda", C.c_int32),
         ("lambda_", C.POINTER(C.c_double)), ("n_refr", C.POINTER(C.c_double)), ("z", C.c_double),
         ("loss", C.c_int), ("prefilter_sigma_px", C.c_double), ("flags", C.c_uint32),
+        ("tuning", C.POINTER(dop_tuning)),
     ]
+
+
+def make_tuning(xdigits: Sequence[int] = (), ydigits: Sequence[int] = (), **fields) -> dop_tuning:
+    """dop_tuning from keyword arguments (marshalling only): xdigits / ydigits = forced digit
+    decompositions, every other keyword is the struct field of that name (include/dop.h)."""
+    t = dop_tuning()
+    t.n_xdigits, t.n_ydigits = len(xdigits), len(ydigits)
+    for i, v in enumerate(xdigits):
+        t.xdigits[i] = int(v)
+    for i, v in enumerate(ydigits):
+        t.ydigits[i] = int(v)
+    for k, v in fields.items():
+        if k not in dict(dop_tuning._fields_) or k in ("reserved", "n_xdigits", "n_ydigits"):
+            raise TypeError(f"dop_tuning has no field {k!r}")
+        setattr(t, k, int(v))
+    return t
 
 
 class DopError(RuntimeError):
@@ -88,13 +114,15 @@ def _ptr(t: Optional[torch.Tensor], dtype, what: str) -> Optional[int]:
 
 
 def dop_plan_create(ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
-                    z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0):
+                    z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0,
+                    tuning: Optional[dop_tuning] = None):
     """-> (plan handle, workspace_bytes).  Host-only; raises DopError on a bad description."""
     nl = len(lambdas)
     lam = (C.c_double * max(nl, 1))(*[float(v) for v in lambdas])
     nr = (C.c_double * max(nl, 1))(*[float(v) for v in n_refr])
     d = dop_plan_desc(int(ny), int(nx), float(pitch), nl, lam, nr, float(z), int(loss),
-                      float(prefilter_sigma_px), int(flags))
+                      float(prefilter_sigma_px), int(flags),
+                      C.pointer(tuning) if tuning is not None else None)
     out, ws = C.c_void_p(), C.c_size_t(0)
     st = _lib.dop_plan_create(C.byref(out), C.byref(d), C.byref(ws))
     if st != DOP_OK:
@@ -165,10 +193,10 @@ class Plan:
 
     def __init__(self, ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
                  z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0,
-                 device: str = "cuda:0"):
+                 device: str = "cuda:0", tuning: Optional[dop_tuning] = None):
         self.ny, self.nx, self.n_lambda, self.loss, self.flags = int(ny), int(nx), len(lambdas), loss, flags
         self.handle, self.workspace_bytes = dop_plan_create(ny, nx, pitch, lambdas, n_refr, z, loss,
-                                                            prefilter_sigma_px, flags)
+                                                            prefilter_sigma_px, flags, tuning)
         self.device = torch.device(device)
         self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
         self.launches = dop_plan_launch_count(self.handle)

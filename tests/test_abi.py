@@ -129,17 +129,18 @@ def test_no_cpu_fallback_without_a_device():
         dop.dop_plan_destroy(plan)
 
 
-def test_launch_count_follows_the_slab_schedule(monkeypatch):
+def _digits(text):
+    return tuple(int(v) for v in text.split(","))
+
+
+def test_launch_count_follows_the_slab_schedule():
     """dop_plan_launch_count is exact for whole-array launches and for the slab schedule."""
     args = (1024, 2048, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0)
-    monkeypatch.setenv("DOP_XDIGITS", "16,128")
-    monkeypatch.delenv("DOP_SLAB_MB", raising=False)
-    h, _ = dop.dop_plan_create(*args)
+    h, _ = dop.dop_plan_create(*args, tuning=dop.make_tuning(xdigits=(16, 128)))
     base = dop.dop_plan_launch_count(h)
     dop.dop_plan_destroy(h)
     assert base == 13 + 1  # 13 passes (x 16.128, y 32.32) + the loss reduction
-    monkeypatch.setenv("DOP_SLAB_MB", "1")
-    h, _ = dop.dop_plan_create(*args)
+    h, _ = dop.dop_plan_create(*args, tuning=dop.make_tuning(xdigits=(16, 128), slab_mb=1))
     n = dop.dop_plan_launch_count(h)
     dop.dop_plan_destroy(h)
     # x segments: rows of 16 KiB -> 64 rows per slab -> 16 slabs; y segments: columns of 8 KiB -> 128 -> 16 slabs
@@ -152,12 +153,63 @@ def test_launch_count_follows_the_slab_schedule(monkeypatch):
     (6144, 128, "384,16", "128", ["y0 L=384 tile=32x384 col pow2", "x0 L=128 tile=32x128 row pow2"]),
     (64, 8192, "64", "8192", ["x0 L=8192 tile=1x8192 row pow2", "y0 L=64 tile=16x64 col pow2"]),
 ])
-def test_plan_routes_digits_to_the_specialised_kernels(ny, nx, yd, xd, expect, monkeypatch):
+def test_plan_routes_digits_to_the_specialised_kernels(ny, nx, yd, xd, expect):
     """dop_plan_describe names, per pass, the tile shape and the kernel family the plan chose."""
-    monkeypatch.setenv("DOP_YDIGITS", yd)
-    monkeypatch.setenv("DOP_XDIGITS", xd)
-    h, _ = dop.dop_plan_create(ny, nx, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0)
+    h, _ = dop.dop_plan_create(ny, nx, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0,
+                               tuning=dop.make_tuning(xdigits=_digits(xd), ydigits=_digits(yd), no_cluster=1))
     text = dop.dop_plan_describe(h)
     dop.dop_plan_destroy(h)
     for e in expect:
         assert e in text, (e, text)
+
+
+def test_the_library_reads_no_environment_variable(monkeypatch):
+    """dop.h: no ambient state.  The round-1 environment knobs must be inert; tuning is explicit."""
+    args = (1024, 2048, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0)
+    h, _ = dop.dop_plan_create(*args)
+    ref = dop.dop_plan_describe(h)
+    dop.dop_plan_destroy(h)
+    for k, v in (("DOP_XDIGITS", "16,128"), ("DOP_YDIGITS", "4,256"), ("DOP_FORCE_GENERIC", "1"), ("DOP_COL_NB", "64"),
+                 ("DOP_SLAB_MB", "1"), ("DOP_TILE_PTS", "256"), ("DOP_H_FLOAT", "1"), ("DOP_PREFETCH_WAVES", "7")):
+        monkeypatch.setenv(k, v)
+    h, _ = dop.dop_plan_create(*args)
+    assert dop.dop_plan_describe(h) == ref
+    dop.dop_plan_destroy(h)
+    src = os.path.join(ROOT, "paper_2505_22313_b200", "csrc")
+    for f in os.listdir(src):
+        assert "getenv" not in open(os.path.join(src, f)).read(), f
+
+
+@pytest.mark.parametrize("tun,status", [
+    (dict(xdigits=(16, 100)), dop.DOP_ERR_UNSUPPORTED_SIZE),        # product != nx
+    (dict(xdigits=(2, 1024)), None),                                # fine: 2 x 1024
+    (dict(xdigits=(1024, 2)), dop.DOP_ERR_UNSUPPORTED_SIZE),        # a non-last x digit is limited to 512
+    (dict(ydigits=(1024,)), dop.DOP_ERR_UNSUPPORTED_SIZE),          # y digits are limited to 512
+    (dict(col_nb=48), dop.DOP_ERR_INVALID_ARG),
+    (dict(tile_pts=100), dop.DOP_ERR_INVALID_ARG),
+    (dict(prefetch_waves=65), dop.DOP_ERR_INVALID_ARG),
+])
+def test_tuning_is_validated(tun, status):
+    """A forced decomposition obeys the same limits as the automatic split: the launch
+    can then never ask for more shared memory than a CTA has."""
+    args = (1024, 2048, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0)
+    if status is None:
+        h, _ = dop.dop_plan_create(*args, tuning=dop.make_tuning(**tun))
+        dop.dop_plan_destroy(h)
+        return
+    with pytest.raises(dop.DopError) as e:
+        dop.dop_plan_create(*args, tuning=dop.make_tuning(**tun))
+    assert e.value.status == status
+
+
+def test_loss_scratch_matches_the_launched_loss_pass():
+    """ADVICE r1 (medium): with a forced column bundle width the loss pass launches fewer, wider CTAs;
+    the scratch and the final reduce must count the CTAs actually launched."""
+    for nb, ctas in ((0, 512), (32, 256), (64, 128)):
+        h, _ = dop.dop_plan_create(64, 16384, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0,
+                                   tuning=dop.make_tuning(xdigits=(128, 128), col_nb=nb, no_cluster=1))
+        text = dop.dop_plan_describe(h)
+        dop.dop_plan_destroy(h)
+        line = [l for l in text.splitlines() if "loss,seed" in l][0]
+        assert f"ctas={ctas} " in line, line
+        assert f"loss_tiles={ctas}" in text, text

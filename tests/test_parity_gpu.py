@@ -27,11 +27,16 @@ def check(a, b, what):
     return e2, ep
 
 
-def run_l2(cfg, h, T, lambdas=None, n_refr=None, write_i=True):
+def digits(text):
+    return tuple(int(v) for v in text.split(","))
+
+
+def run_l2(cfg, h, T, lambdas=None, n_refr=None, write_i=True, tuning=None):
     lambdas = cfg.lambdas if lambdas is None else lambdas
     n_refr = cfg.n_refr if n_refr is None else n_refr
     flags = dop.DOP_WRITE_INTENSITY if write_i else 0
-    plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, lambdas, n_refr, cfg.z, dop.DOP_LOSS_L2, cfg.sigma_px, flags, DEV)
+    plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, lambdas, n_refr, cfg.z, dop.DOP_LOSS_L2, cfg.sigma_px, flags, DEV,
+                    tuning=tuning)
     inten = torch.full((len(lambdas), cfg.ny, cfg.nx), float("nan"), dtype=torch.float32, device=DEV) if write_i else None
     grad = torch.full_like(h, float("nan"))
     loss = torch.full((1,), float("nan"), dtype=torch.float64, device=DEV)
@@ -111,16 +116,12 @@ def test_prefilter_path(ny, nx):
     assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
 
 
-@pytest.mark.parametrize("env", [{"DOP_XDIGITS": "16,8", "DOP_YDIGITS": "4,12"},
-                                 {"DOP_XDIGITS": "2,4,16", "DOP_YDIGITS": "3,4,4"},
-                                 {"DOP_XDIGITS": "128", "DOP_YDIGITS": "48"}])
-def test_every_digit_decomposition_gives_the_same_answer(env, monkeypatch):
+@pytest.mark.parametrize("xd,yd", [("16,8", "4,12"), ("2,4,16", "3,4,4"), ("128", "48")])
+def test_every_digit_decomposition_gives_the_same_answer(xd, yd):
     """The multi-pass (four-step) decomposition used for 65536-point lines, forced on a small grid."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
     cfg = synth.CONFIGS["C5"].scaled(48, 128)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
-    I, L, g = run_l2(cfg, h, T)
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(xdigits=digits(xd), ydigits=digits(yd)))
     Ir, Lr, gr = oracle_l2(cfg, h, T)
     check(I, Ir, "intensity")
     check(g, gr, "dL/dh")
@@ -151,31 +152,30 @@ KERNEL_FAMILIES = [
 ]
 
 
+@pytest.mark.parametrize("generic", [0, 1])
 @pytest.mark.parametrize("ny,nx,yd,xd", KERNEL_FAMILIES)
-def test_every_kernel_family_against_the_oracle(ny, nx, yd, xd, monkeypatch):
+def test_every_kernel_family_against_the_oracle(ny, nx, yd, xd, generic):
     """Forces digit decompositions so that each instantiated digit length of the register-blocked
     kernels (column tile / H / per-lane variants, staged and unstaged row tiles, 3 x 2^k) runs the
-    fused L2 path and is compared with the oracle."""
-    monkeypatch.setenv("DOP_YDIGITS", yd)
-    monkeypatch.setenv("DOP_XDIGITS", xd)
+    fused L2 path and is compared with the oracle; generic = 1 runs the same plans on the generic
+    shared-memory kernel (force_generic), i.e. that kernel at full digit lengths."""
     cfg = synth.CONFIGS["C4"].scaled(ny, nx)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
-    I, L, g = run_l2(cfg, h, T)
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(xdigits=digits(xd), ydigits=digits(yd), force_generic=generic,
+                                                      no_cluster=1))
     Ir, Lr, gr = oracle_l2(cfg, h, T)
     check(I, Ir, "intensity")
     check(g, gr, "dL/dh")
     assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
 
 
-def test_slab_schedule_gives_the_same_answer(monkeypatch):
-    """DOP_SLAB_MB: multi-pass segments run slab by slab on auxiliary streams (fork / join on the
+def test_slab_schedule_gives_the_same_answer():
+    """dop_tuning.slab_mb: multi-pass segments run slab by slab on auxiliary streams (fork / join on the
     caller's stream); 1 MiB slabs split this grid into 16 column slabs and 16 row slabs."""
-    monkeypatch.setenv("DOP_XDIGITS", "16,128")
     cfg = synth.CONFIGS["C4"].scaled(1024, 2048)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
-    I0, L0, g0 = run_l2(cfg, h, T)
-    monkeypatch.setenv("DOP_SLAB_MB", "1")
-    I1, L1, g1 = run_l2(cfg, h, T)
+    I0, L0, g0 = run_l2(cfg, h, T, tuning=dop.make_tuning(xdigits=(16, 128)))
+    I1, L1, g1 = run_l2(cfg, h, T, tuning=dop.make_tuning(xdigits=(16, 128), slab_mb=1))
     # same kernels on the same tiles, only the launch grouping differs: bit-identical
     assert np.array_equal(I0, I1) and np.array_equal(g0, g1) and L0 == L1
     Ir, Lr, gr = oracle_l2(cfg, h, T)
@@ -184,17 +184,15 @@ def test_slab_schedule_gives_the_same_answer(monkeypatch):
     assert abs(L1 - Lr) <= TOL_LOSS * abs(Lr)
 
 
-@pytest.mark.parametrize("z,env", [(2e-3, {"DOP_H_FLOAT": "1"}), (0.4, {}), (-0.4, {}), (0.28, {})])
-def test_both_phase_paths_of_H(z, env, monkeypatch):
+@pytest.mark.parametrize("z,h_float", [(2e-3, 1), (0.4, 0), (-0.4, 0), (0.28, 0), (0.28, 1)])
+def test_both_phase_paths_of_H(z, h_float):
     """H's phase is taken in 32-bit fixed point while |z|/lambda < 2^19 turns and through the fp32
-    fraction otherwise (or with DOP_H_FLOAT): both against the oracle, on both sides of the switch
-    (0.28 m / 550 nm = 509 091 turns < 2^19 = 524 288 <= 0.4 m / 550 nm)."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+    fraction otherwise (or with dop_tuning.h_float): both against the oracle, on both sides of the
+    switch (0.28 m / 550 nm = 509 091 turns < 2^19 = 524 288 <= 0.4 m / 550 nm)."""
     import dataclasses
     cfg = dataclasses.replace(synth.CONFIGS["C4"].scaled(512, 256), z=z)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
-    I, L, g = run_l2(cfg, h, T)
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(h_float=h_float))
     Ir, Lr, gr = oracle_l2(cfg, h, T)
     check(I, Ir, "intensity")
     check(g, gr, "dL/dh")
@@ -286,15 +284,13 @@ def test_repeatable_bitwise():
     (65536, 32, "256,256", "32"),    # 32-column bundles
     (6144, 128, "384,16", "128"),    # 3 x 128
 ])
-def test_repeatable_bitwise_under_load(ny, nx, yd, xd, monkeypatch):
+def test_repeatable_bitwise_under_load(ny, nx, yd, xd):
     """A missing barrier (the row kernels synchronise most exchanges with __syncwarp only) would show
     as run-to-run differences: the full grid keeps every SM busy with several CTAs, 8 repeats."""
-    monkeypatch.setenv("DOP_YDIGITS", yd)
-    monkeypatch.setenv("DOP_XDIGITS", xd)
     cfg = synth.CONFIGS["C4"].scaled(ny, nx)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
     plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, 0.0,
-                    dop.DOP_WRITE_INTENSITY, DEV)
+                    dop.DOP_WRITE_INTENSITY, DEV, tuning=dop.make_tuning(xdigits=digits(xd), ydigits=digits(yd)))
     inten = torch.empty((1, ny, nx), dtype=torch.float32, device=DEV)
     grad = torch.empty_like(h)
     loss = torch.zeros(1, dtype=torch.float64, device=DEV)
