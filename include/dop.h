@@ -86,10 +86,16 @@ typedef struct {
     int32_t slab_streams;   /* 1..4 auxiliary streams of the slab schedule (0 = default 2)              */
     int32_t h_float;        /* != 0: take the phase of H through an fp32 fraction, never fixed point    */
     int32_t tile_pts;       /* 256..16384: tile size of the generic kernel (0 = default 4096)           */
-    int32_t no_cluster;     /* != 0: never use the thread-block-cluster row kernels (long x axes then   */
-                            /*       run as two digit passes)                                           */
+    int32_t no_cluster;     /* != 0: never use the thread-block-cluster row kernels (cluster_row.cuh)   */
     int32_t no_mirror;      /* != 0: do not pair mirrored ky tiles in the (x) H pass                    */
-    int32_t reserved[7];    /* must be 0                                                                */
+    int32_t cluster_dsmem;  /* != 0: the cluster row kernels exchange through distributed shared memory  */
+                            /*       instead of through L2 (measured slower on B200; kept as evidence)   */
+    int32_t cluster_lines;  /* 1 | 2 | 4 | 8: lines per CTA of the cluster row kernels, i.e. cluster size   */
+                            /*       16 / lines (0 = default: 512-thread CTAs)                           */
+    int32_t cluster_force;  /* != 0: cluster row kernels wherever they exist (nx = 16384, 32768, 65536);  */
+                            /*       by default only where measured faster than two digit passes          */
+                            /*       (nx = 16384, clusters of 2; profiles/r02_cluster.md)                 */
+    int32_t reserved[4];    /* must be 0                                                                */
 } dop_tuning;
 
 typedef struct {

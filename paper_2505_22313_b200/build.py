@@ -22,7 +22,8 @@ SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu"]
 POW2_INST = [(1, L) for L in (16, 32, 64, 128, 256, 512)] + \
             [(0, L) for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192)]
 POW2_X3 = (16, 32, 64, 128)  # digits 3 * LP
-HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", os.path.join("..", "..", "include", "dop.h")]
+CLUSTER_INST = [(4096, 2), (4096, 1), (2048, 4), (1024, 8)]  # (local transform length M, lines per CTA S): rows of 16 M
+HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", "cluster_row.cuh", os.path.join("..", "..", "include", "dop.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC",
@@ -39,6 +40,9 @@ def _nvcc() -> str:
 def _units():
     """(object path, source path, extra flags) of every translation unit."""
     units = [(os.path.join(OBJDIR, s.replace(".cu", ".o")), os.path.join(CSRC, s), []) for s in SOURCES]
+    for m, sl in CLUSTER_INST:
+        units.append((os.path.join(OBJDIR, f"cluster_{m}_{sl}.o"), os.path.join(CSRC, "cluster_inst.cu"),
+                      [f"-DDOP_INST_CLUSTER_M={m}", f"-DDOP_INST_CLUSTER_S={sl}"]))
     for lp in POW2_X3:
         units.append((os.path.join(OBJDIR, f"pow2_x3_{lp}.o"), os.path.join(CSRC, "pow2_inst.cu"),
                       [f"-DDOP_INST_X3={lp}"]))
@@ -50,7 +54,7 @@ def _units():
 
 def _dep_stamp() -> str:
     h = hashlib.sha256()
-    for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS + ["pow2_inst.cu"]] + [os.path.abspath(__file__)]:
+    for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS + ["pow2_inst.cu", "cluster_inst.cu"]] + [os.path.abspath(__file__)]:
         with open(d, "rb") as f:
             h.update(f.read())
     h.update((" ".join(NVCC_FLAGS) + os.environ.get("DOP_NVCC_EXTRA", "")).encode())

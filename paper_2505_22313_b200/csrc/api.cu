@@ -107,7 +107,8 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
 {
     PassDesc d{};
     pass_geometry(p, t, &d);
-    const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
+    // (a cluster pass takes its group twiddles from x digit 1 and its boundary twiddles from x digit 0)
+    const Digit& g = p->ax[t.axis].dig[(size_t)(t.cluster ? 1 : t.digit)];
     char* arena = (char*)p->d_arena;
     const size_t npts = (size_t)p->desc.nx * (size_t)p->desc.ny;
     d.fft1_dir = t.fft1_dir;
@@ -117,6 +118,12 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.tw_b = g.has_twb ? (const float2*)(arena + g.twb_off) : nullptr;
     d.tw_b2 = g.twb2.empty() ? nullptr : (const float2*)(arena + g.twb2_off);
     d.twb_n = g.L * g.st;
+    if (t.cluster) {
+        const Digit& g0 = p->ax[0].dig[0];
+        d.tw_b = nullptr;
+        d.tw_b2 = (const float2*)(arena + g0.twb2_off);
+        d.twb_n = g0.L * g0.st;
+    }
     d.tw_g = g.fast ? (const float2*)(arena + g.twg_off) : nullptr;
     d.load_op = t.load_op;
     d.mid_op = t.mid_op;
@@ -150,13 +157,13 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.h_fixed = (std::fabs(p->desc.z) / lambda < 524288.0 && !p->h_float) ? 1 : 0;
     // prefetch distance in tiles: pf_waves x (148 SMs x resident CTAs of ~1024 threads per SM)
     {
-        const long long threads = d.col_type ? d.L : (long long)d.nl * d.L / 16;
+        const long long threads = d.cluster ? 512 : (d.col_type ? d.L : (long long)d.nl * d.L / 16);
         const long long per_sm = threads > 0 ? (1024 / threads > 0 ? 1024 / threads : 1) : 1;
         d.pf_ahead = (int)(p->pf_waves * 148 * per_sm);
         // Measured (C2 / C3 / C4): a gain on row-type tiles (C3 x passes 0.86 -> 0.75 ms, C2 loss pass
         // 0.57 -> 0.52 ms); on column tiles a loss, or a wash that over-fetches DRAM by 15-50 %
         // (ncu) -- with 32-column bundles the C2 y passes run 0.217 ms with it and 0.204 ms without.
-        if (d.col_type) d.pf_ahead = 0;
+        if (d.col_type || d.cluster) d.pf_ahead = 0;
     }
     d.device = p->device;
     d.fx2 = p->d_f2[0];
@@ -219,6 +226,7 @@ bool slab_layout(const dop_plan* p, const std::vector<D>& d, int axis, long long
 
 std::string pass_label(const char* tag, const PassTmpl& t)
 {
+    if (t.cluster) return std::string(tag) + ":x0+x1:" + t.name;
     return std::string(tag) + ":" + (t.axis == 0 ? "x" : "y") + std::to_string(t.digit) + ":" + t.name;
 }
 

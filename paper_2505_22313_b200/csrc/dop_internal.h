@@ -95,12 +95,16 @@ struct PassDesc {
     long long row_o, row_m, row_i; // y slot of element i: o*row_o + m*row_m + i*row_i
     int smem_bytes;
     int threads;
+    int cluster;          // 1 (exchange through L2) | 2 (through DSMEM) = cluster row pass (cluster_row.cuh): L = M, the x digits (16, M) fused; n_o rows
     int device;           // the plan's device (function attributes are set once per device)
 };
 
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream);
 // register-blocked power-of-two fast path (kernels_pow2.cu)
 bool pow2_supported(long long L, bool col_type);
+bool cluster_supported(long long L0, long long L1);
+int cluster_size(long long L1);
+bool cluster_instantiated(long long L1, int lines);
 int pow2_lines(long long L, bool col_type, bool plain = false, int nb_override = 0);
 std::vector<float2> pow2_group_twiddles(long long L);
 cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
@@ -143,6 +147,7 @@ struct PassTmpl {
     std::string name;
     double bytes_per_point; // algorithmic HBM bytes per grid point of this launch
     double rd, wr, side;    // its parts: main input read, main output written, side planes (T, I, h, grad)
+    int cluster = 0;        // x digits (16, M) fused into one thread-block-cluster pass
 };
 
 } // namespace dop
@@ -161,7 +166,8 @@ struct dop_plan {
     int slab_streams = 2;       // DOP_SLAB_STREAMS
     int pf_waves = 1;           // L2 prefetch distance of the pow2 kernels, in waves of resident CTAs (0 = off)
     long long slab_bytes = 0;   // L2 slab size for multi-pass segments (0 = whole-array launches)
-    bool force_generic = false; // DOP_FORCE_GENERIC at plan creation: generic kernel for every pass
+    bool force_generic = false; // dop_tuning.force_generic: generic kernel for every pass
+    bool x_cluster = false;     // the x digits are (16, M) and run as one cluster pass
     // schedules for one lambda
     std::vector<dop::PassTmpl> fwd, adj, pre; // pre = Gaussian pre-filter (real -> real)
     long long loss_tiles = 0;                 // CTAs of the MID_LOSS pass

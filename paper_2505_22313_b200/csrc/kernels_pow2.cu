@@ -2,9 +2,14 @@
 // (pow2_impl.cuh; instantiated per digit length in pow2_inst.cu) and their host-side tables.
 #include <cstdlib>
 
-#include "pow2_impl.cuh"
+#include "cluster_row.cuh"
 
 namespace dop {
+
+extern template cudaError_t launch_cluster<4096, 2>(const PassDesc&, int, cudaStream_t);
+extern template cudaError_t launch_cluster<4096, 1>(const PassDesc&, int, cudaStream_t);
+extern template cudaError_t launch_cluster<2048, 4>(const PassDesc&, int, cudaStream_t);
+extern template cudaError_t launch_cluster<1024, 8>(const PassDesc&, int, cudaStream_t);
 
 // explicit instantiations live in the pow2_inst.cu objects
 #define DOP_DECL(L, COL) extern template cudaError_t launch_L<L, COL>(const PassDesc&, int, int, cudaStream_t);
@@ -64,9 +69,35 @@ static int pass_variant(const PassDesc& p)
     return V_STOTHER; // ST_C64_INTENSITY, ST_REAL
 }
 
+// x axes of 16 M points (M = 1024, 2048, 4096) can run their two digit passes (16, M) as one
+// thread-block-cluster pass (cluster_row.cuh)
+bool cluster_supported(long long L0, long long L1) { return L0 == 16 && (L1 == 1024 || L1 == 2048 || L1 == 4096); }
+int cluster_size(long long L1) { return L1 == 4096 ? 8 : (L1 == 2048 ? 4 : 2); }
+bool cluster_instantiated(long long L1, int lines)
+{
+    return (L1 == 4096 && (lines == 2 || lines == 1)) || (L1 == 2048 && lines == 4) || (L1 == 1024 && lines == 8);
+}
+
+static cudaError_t launch_cluster_pass(const PassDesc& p, cudaStream_t stream)
+{
+    const int v = pass_variant(p);
+    if (v < 0 || p.tw_g == nullptr || p.tw_b2 == nullptr) return cudaErrorInvalidValue;
+    switch (p.L * 16 + p.nl) {
+    case 4096 * 16 + 2: return launch_cluster<4096, 2>(p, v, stream);
+    case 4096 * 16 + 1: return launch_cluster<4096, 1>(p, v, stream);
+    case 2048 * 16 + 4: return launch_cluster<2048, 4>(p, v, stream);
+    case 1024 * 16 + 8: return launch_cluster<1024, 8>(p, v, stream);
+    }
+    return cudaErrorInvalidValue;
+}
+
 cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* handled)
 {
     *handled = false;
+    if (p.cluster) { // a cluster pass has no other implementation: the plan only schedules supported ones
+        *handled = true;
+        return launch_cluster_pass(p, stream);
+    }
     const bool col = p.col_type != 0;
     if (p.tw_g == nullptr || !pow2_supported(p.L, col)) return cudaSuccess;
     if (col ? !(p.nl == 16 || p.nl == 32 || p.nl == 64) : p.nl != pow2_lines(p.L, false)) return cudaSuccess;

@@ -186,7 +186,7 @@ static PassTmpl mk(int axis, int digit, int d1, int d2, int ld, int mid, int st,
 // passes of  F^-1{ mid (x) F{.} }  minus the first forward x digit and the last inverse x digit
 static void sandwich_core(const dop_plan* p, int mid, bool with_xfwd, std::vector<PassTmpl>* out)
 {
-    const int a = (int)p->ax[0].dig.size(), b = (int)p->ax[1].dig.size();
+    const int a = p->x_cluster ? 1 : (int)p->ax[0].dig.size(), b = (int)p->ax[1].dig.size();
     if (with_xfwd)
         for (int j = 1; j < a; ++j) out->push_back(mk(0, j, +1, 0, LD_C64, MID_NONE, ST_C64, "x-fwd", 8, 8));
     for (int j = 0; j + 1 < b; ++j) out->push_back(mk(1, j, +1, 0, LD_C64, MID_NONE, ST_C64, "y-fwd", 8, 8));
@@ -200,7 +200,8 @@ static void build_schedule(dop_plan* p)
 {
     const bool l2 = p->desc.loss == DOP_LOSS_L2;
     const bool wi = l2 && (p->desc.flags & DOP_WRITE_INTENSITY);
-    const int a = (int)p->ax[0].dig.size();
+    // with cluster row passes the x digits (16, M) always run fused: one x pass per transform pair
+    const int a = p->x_cluster ? 1 : (int)p->ax[0].dig.size();
     p->fwd.clear(); p->adj.clear(); p->pre.clear();
     // forward
     p->fwd.push_back(mk(0, 0, +1, 0, LD_HEIGHT, MID_NONE, ST_C64, "h->u0,x-fwd", 4, 8));
@@ -224,6 +225,10 @@ static void build_schedule(dop_plan* p)
         sandwich_core(p, MID_GAUSS, true, &p->pre);
         p->pre.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_REAL, "x-inv,real", 8, 4));
     }
+    if (p->x_cluster)
+        for (std::vector<PassTmpl>* v : {&p->fwd, &p->adj, &p->pre})
+            for (PassTmpl& t : *v)
+                if (t.axis == 0) t.cluster = 1;
 }
 
 void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
@@ -274,6 +279,23 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
 // variants stay at 16 columns.
 void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d)
 {
+    if (t.cluster) { // one cluster of C CTAs per row; CTA = S lines of M points
+        const long long M = p->ax[0].dig[1].L;
+        const int C = p->tune.cluster_lines > 0 ? 16 / p->tune.cluster_lines : cluster_size(M);
+        *d = PassDesc{};
+        d->cluster = p->tune.cluster_dsmem ? 2 : 1;
+        d->L = (int)M;
+        d->nl = 16 / C;
+        d->col_type = 0;
+        d->es = 1;
+        d->NC = C; d->SCc = 0;
+        d->n_cgroups = C;
+        d->n_m = 1; d->SM = 0;
+        d->n_o = p->desc.ny; d->SO = p->desc.nx;
+        d->smem_bytes = (int)((16 / C) * (M + 2 * (M / 32)) * (long long)sizeof(float2));
+        d->threads = (int)((16 / C) * (M / 16));
+        return;
+    }
     tile_geometry(p, t.axis, t.digit, d);
     const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
     if (!g.fast || !d->col_type) return;
@@ -313,14 +335,27 @@ dop_status build_plan(dop_plan* p)
     // default: measured slower than whole-array launches on B200.
     if (tu.slab_mb < 0 || tu.slab_mb > 4096) return DOP_ERR_INVALID_ARG;
     p->slab_bytes = (long long)tu.slab_mb << 20;
-    for (int i = 0; i < 7; ++i)
+    for (int i = 0; i < 4; ++i)
         if (tu.reserved[i] != 0) return DOP_ERR_INVALID_ARG;
+    if (tu.cluster_lines != 0 && tu.cluster_lines != 1 && tu.cluster_lines != 2 && tu.cluster_lines != 4 && tu.cluster_lines != 8)
+        return DOP_ERR_INVALID_ARG;
     // generic kernel limits: a row-type line <= 8192 points (64 KiB), a column-type digit
     // <= 512 points (x 16 adjacent lines = 64 KiB)
     std::vector<long long> lx, ly;
-    if (!split_digits(d.nx, 512, 8192, tu.n_xdigits, tu.xdigits, &lx)) return DOP_ERR_UNSUPPORTED_SIZE;
+    // Cluster row passes: measured on B200 a gain for clusters of 2 (nx = 16384: C3 +7 %), a loss of
+    // 5-15 % against two digit passes for clusters of 4-16 (profiles/r02_cluster.md), so only the
+    // former is a default; dop_tuning.cluster_force selects them wherever they exist.
+    const bool may_cluster = !tu.no_cluster && !p->force_generic;
+    const bool want_cluster = may_cluster && d.nx % 16 == 0 && cluster_supported(16, d.nx / 16) &&
+                              (tu.cluster_force || d.nx == 16384);
+    if (want_cluster && tu.n_xdigits == 0) {
+        lx = {16, d.nx / 16}; // rows of 16 M points: one thread-block-cluster pass per transform pair
+    } else if (!split_digits(d.nx, 512, 8192, tu.n_xdigits, tu.xdigits, &lx)) return DOP_ERR_UNSUPPORTED_SIZE;
     if (!split_digits(d.ny, 512, 512, tu.n_ydigits, tu.ydigits, &ly)) return DOP_ERR_UNSUPPORTED_SIZE;
     if (!build_axis(p, 0, d.nx, lx) || !build_axis(p, 1, d.ny, ly)) return DOP_ERR_UNSUPPORTED_SIZE;
+    p->x_cluster = want_cluster && lx.size() == 2 && cluster_supported(lx[0], lx[1]) && p->ax[0].dig[0].fast &&
+                   p->ax[0].dig[1].fast;
+    if (p->x_cluster && tu.cluster_lines > 0 && !cluster_instantiated(lx[1], tu.cluster_lines)) return DOP_ERR_INVALID_ARG;
     build_schedule(p);
     // CTAs of the MID_LOSS pass, in the geometry it is launched with (one loss partial per CTA)
     p->loss_tiles = 0;
@@ -364,8 +399,12 @@ std::string describe_plan(const dop_plan* p)
         for (const PassTmpl& t : v) {
             PassDesc g{};
             pass_geometry(p, t, &g);
-            os << tag << " " << (t.axis == 0 ? "x" : "y") << t.digit << " L=" << g.L << " tile=" << g.nl << "x" << g.L
-               << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? " pow2" : " generic") << " ctas=" << g.n_cgroups * g.n_m * g.n_o
+            if (t.cluster)
+                os << tag << " x0+x1 L=16x" << g.L << " tile=" << g.nl << "x" << g.L << " row cluster=" << g.n_cgroups;
+            else
+                os << tag << " " << (t.axis == 0 ? "x" : "y") << t.digit << " L=" << g.L << " tile=" << g.nl << "x" << g.L
+                   << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? " pow2" : " generic");
+            os << " ctas=" << g.n_cgroups * g.n_m * g.n_o
                << " smem=" << g.smem_bytes << " B/pt=" << t.bytes_per_point << " [" << t.name << "]\n";
             total += t.bytes_per_point;
         }

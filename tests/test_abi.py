@@ -163,6 +163,25 @@ def test_plan_routes_digits_to_the_specialised_kernels(ny, nx, yd, xd, expect):
         assert e in text, (e, text)
 
 
+def test_cluster_row_passes_in_the_plan():
+    """Rows of 16 M points can run their x digit pair (16, M) as ONE thread-block-cluster pass (one read
+    + one write of the field per x transform pair).  Default where measured faster (nx = 16384, clusters
+    of 2: config 3); dop_tuning.cluster_force selects them at 65536 too: 144 instead of 208 B/point."""
+    h, _ = dop.dop_plan_create(16384, 16384, 0.25e-6, (550e-9,), (1.5,), 0.01)
+    text = dop.dop_plan_describe(h)
+    dop.dop_plan_destroy(h)
+    assert "x0+x1 L=16x1024 tile=8x1024 row cluster=2" in text and "algorithmic_bytes_per_point=144" in text, text
+    h, _ = dop.dop_plan_create(98304, 65536, 0.25e-6, (550e-9,), (1.5,), 0.1)
+    text = dop.dop_plan_describe(h)
+    dop.dop_plan_destroy(h)
+    assert "cluster" not in text and "algorithmic_bytes_per_point=208" in text, text
+    h, _ = dop.dop_plan_create(98304, 65536, 0.25e-6, (550e-9,), (1.5,), 0.1, tuning=dop.make_tuning(cluster_force=1))
+    text = dop.dop_plan_describe(h)
+    assert dop.dop_plan_launch_count(h) == 9 + 1
+    dop.dop_plan_destroy(h)
+    assert "x0+x1 L=16x4096 tile=2x4096 row cluster=8" in text and "algorithmic_bytes_per_point=144" in text, text
+
+
 def test_the_library_reads_no_environment_variable(monkeypatch):
     """dop.h: no ambient state.  The round-1 environment knobs must be inert; tuning is explicit."""
     args = (1024, 2048, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0)

@@ -146,6 +146,24 @@ def test_sinusoidal_phase_grating_jacobi_anger():
     assert 1 / lam ** 2 < (K * a / (nx * pitch)) ** 2
 
 
+def test_phase_grating_closed_form_with_aliased_orders():
+    """The evaluator the GPU suite uses at C4 / C5 size (tests/closed_forms.py): grating frequencies so high
+    that most orders alias (k a > nx/2) and a good part of them is evanescent; against the oracle at every
+    point of a small grid."""
+    from closed_forms import grating_field, grating_phase
+    ny, nx, pitch, lam, n, z = 96, 128, 0.25e-6, 550e-9, 1.5, 0.3e-3
+    a, b, m1, m2 = 37, 29, 1.8, 1.3
+    c = m1 + m2
+    y, x = np.mgrid[0:ny, 0:nx]
+    h = grating_phase(ny, nx, a, b, m1, m2, c, y, x) * lam / (2 * np.pi * (n - 1))
+    assert h.min() >= 0 and h.max() <= 1.1e-6
+    out = orc.forward(h, pitch, [lam], [n], z)
+    ref, Hkl = grating_field(ny, nx, pitch, lam, z, a, b, m1, m2, c, y.ravel(), x.ravel())
+    assert np.abs(out["u"][0].ravel() - ref).max() < 1e-11
+    cut = np.mean(Hkl == 0)
+    assert 0.1 < cut < 0.9          # the evanescent mask is exercised on both sides
+
+
 # ---------------------------------------------------------------------------------- P-k
 def test_periodic_tiling_invariance_forward():
     rng = np.random.default_rng(6)

@@ -169,6 +169,62 @@ def test_every_kernel_family_against_the_oracle(ny, nx, yd, xd, generic):
     assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
 
 
+@pytest.mark.parametrize("ny,nx", [(8, 16384), (6, 32768), (4, 65536), (96, 65536)])
+def test_cluster_row_passes_against_the_oracle(ny, nx):
+    """Rows of 16 M points (M = 1024, 2048, 4096) run their two x digit passes as ONE thread-block-cluster
+    pass (cluster_row.cuh; DSMEM all-to-all between a radix-16 step and the M-point line transforms):
+    fused L2 path, caller-seeded path (field u readable) and pre-filter, all against the oracle, and
+    against the same plan with the cluster kernels switched off (dop_tuning.no_cluster)."""
+    cfg = synth.CONFIGS["C4"].scaled(ny, nx)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    force = dop.make_tuning(cluster_force=1)
+    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, 0.0, 0, DEV, tuning=force)
+    text = plan.describe()
+    plan.close()
+    assert "x0+x1 L=16x%d" % (nx // 16) in text and "row cluster=%d" % {1024: 2, 2048: 4, 4096: 8}[nx // 16] in text
+    I, L, g = run_l2(cfg, h, T, tuning=force)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+    I2, L2, g2 = run_l2(cfg, h, T, tuning=dop.make_tuning(no_cluster=1))
+    I4, L4, g4 = run_l2(cfg, h, T, tuning=dop.make_tuning(cluster_force=1, cluster_dsmem=1))
+    check(I4, Ir, "intensity (DSMEM exchange)")
+    check(g4, gr, "dL/dh (DSMEM exchange)")
+    if nx == 65536:  # clusters of 16 CTAs of 256 threads
+        for dsmem in (0, 1):
+            I5, L5, g5 = run_l2(cfg, h, T, tuning=dop.make_tuning(cluster_force=1, cluster_lines=1, cluster_dsmem=dsmem))
+            check(I5, Ir, "intensity (clusters of 16)")
+            check(g5, gr, "dL/dh (clusters of 16)")
+    check(I2, Ir, "intensity (two digit passes)")
+    check(I, I2, "cluster vs digit passes")
+    check(g, g2, "cluster vs digit passes, dL/dh")
+    # caller-seeded path: field u, I, then adj with dL/dI
+    dLdI = synth.uniform_plane(78, 5, ny, nx, DEV).view(1, ny, nx).contiguous() - 0.5
+    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_NONE, 0.0, 0, DEV, tuning=force)
+    inten = torch.empty((1, ny, nx), dtype=torch.float32, device=DEV)
+    grad = torch.empty_like(h)
+    plan.fwd(h, None, inten, None)
+    torch.cuda.synchronize()
+    u = plan.field().cpu().numpy()
+    plan.adj(h, dLdI, grad)
+    torch.cuda.synchronize()
+    plan.close()
+    hn = h.cpu().numpy()
+    ref = orc.forward(hn, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z)
+    check(u, ref["u"], "field u")
+    check(inten.cpu().numpy(), ref["I"], "intensity (LOSS_NONE)")
+    check(grad.cpu().numpy(), orc.adjoint(hn, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dLdI=dLdI.cpu().numpy()), "dL/dh")
+    # pre-filter (real-plane load / store variants)
+    cfg3 = synth.CONFIGS["C3"].scaled(ny, nx)
+    h3, T3 = synth.make_height(cfg3, DEV), synth.make_target(cfg3, DEV)
+    I3, L3, g3 = run_l2(cfg3, h3, T3, tuning=force)
+    I3r, L3r, g3r = oracle_l2(cfg3, h3, T3)
+    check(I3, I3r, "intensity (pre-filter)")
+    check(g3, g3r, "dL/dh (pre-filter)")
+    assert abs(L3 - L3r) <= TOL_LOSS * abs(L3r)
+
+
 def test_slab_schedule_gives_the_same_answer():
     """dop_tuning.slab_mb: multi-pass segments run slab by slab on auxiliary streams (fork / join on the
     caller's stream); 1 MiB slabs split this grid into 16 column slabs and 16 row slabs."""
@@ -283,6 +339,8 @@ def test_repeatable_bitwise():
     (256, 8192, "16,16", "8192"),    # 8192-point rows (runs of 2 slots, CTA-wide exchanges)
     (65536, 32, "256,256", "32"),    # 32-column bundles
     (6144, 128, "384,16", "128"),    # 3 x 128
+    (2048, 65536, "32,64", "16,4096"),  # cluster row passes (DSMEM exchanges between 8 CTAs)
+    (4096, 16384, "64,64", "16,1024"),  # cluster of 2
 ])
 def test_repeatable_bitwise_under_load(ny, nx, yd, xd):
     """A missing barrier (the row kernels synchronise most exchanges with __syncwarp only) would show
@@ -290,7 +348,8 @@ def test_repeatable_bitwise_under_load(ny, nx, yd, xd):
     cfg = synth.CONFIGS["C4"].scaled(ny, nx)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
     plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, 0.0,
-                    dop.DOP_WRITE_INTENSITY, DEV, tuning=dop.make_tuning(xdigits=digits(xd), ydigits=digits(yd)))
+                    dop.DOP_WRITE_INTENSITY, DEV,
+                    tuning=dop.make_tuning(xdigits=digits(xd), ydigits=digits(yd), cluster_force=1))
     inten = torch.empty((1, ny, nx), dtype=torch.float32, device=DEV)
     grad = torch.empty_like(h)
     loss = torch.zeros(1, dtype=torch.float64, device=DEV)
@@ -409,8 +468,6 @@ def plane_wave_case(name, a, b, p, q, tau=0.25, nsamp=4096):
     rng = np.random.default_rng(11)
     sy, sx = rng.integers(0, ny, nsamp), rng.integers(0, nx, nsamp)
     th = 2 * np.pi * (((p * sx * ny + q * sy * nx) % (nx * ny)) / float(nx * ny))
-    # the fp32-rounded h the GPU saw defines u0; use it for the closed form's u0 phase
-    hs = h[torch.from_numpy(sy).to(DEV), torch.from_numpy(sx).to(DEV)].double().cpu().numpy()
     N = float(nx * ny)
     gref = (2 * np.pi * (n - 1) / lam) * (2 * tau / N) * np.imag(
         H0 * (np.conj(Hp) * np.exp(1j * th) + np.conj(Hm) * np.exp(-1j * th)))
@@ -420,12 +477,11 @@ def plane_wave_case(name, a, b, p, q, tau=0.25, nsamp=4096):
     A, B = H0 * np.conj(Hp), H0 * np.conj(Hm)
     assert np.hypot(A.imag + B.imag, A.real - B.real) >= 0.5, "ill-conditioned plane-wave pin: choose other p, q"
     # loss: I == 1 exactly, so L = mean (tau cos)^2 = tau^2/2
-    assert abs(float(loss.item()) - tau * tau / 2) <= 2e-5 * tau * tau / 2
+    assert abs(float(loss.item()) - tau * tau / 2) <= TOL_LOSS * tau * tau / 2
     e2 = np.linalg.norm(gs - gref) / np.linalg.norm(gref)
     ep = np.abs(gs - gref).max() / np.abs(gref).max()
-    # the closed form assumes h exact; fp32 storage of h perturbs the phase by ~4e-7 rad, below the bar
-    assert e2 <= 2e-5 and ep <= TOL_PEAK, f"{name} plane-wave dL/dh: {e2:.3e} {ep:.3e}"
-    assert hs.min() >= 0
+    # (the closed form assumes the ideal ramp; storing h in fp32 perturbs the phase by ~4e-7 rad, well below the bar)
+    assert e2 <= TOL_L2 and ep <= TOL_PEAK, f"{name} plane-wave dL/dh: {e2:.3e} {ep:.3e}"
     if inten is not None:
         Is = inten[0][torch.from_numpy(sy).to(DEV), torch.from_numpy(sx).to(DEV)].cpu().numpy()
         assert np.abs(Is - 1.0).max() <= 1e-4
@@ -453,3 +509,77 @@ def test_C5_full_size_tiled():
 @HUGE
 def test_C5_full_size_plane_wave_closed_form():
     plane_wave_case("C5", 5001, -3 * 2111, 1234, 3 * 779)
+
+
+@HUGE
+def test_C4_full_size_plane_wave_closed_form():
+    plane_wave_case("C4", 5001, -6333, 1234, 2337)
+
+
+def grating_case(name, a, b, m1=1.8, m2=1.3, nsamp=100000, expect_cut=True):
+    """Pin P-j at full size on the GPU: a two-sinusoid phase grating; the field u
+    (DOP_LOSS_NONE, read from the workspace) against the Jacobi-Anger closed form of
+    tests/closed_forms.py in fp64 at ~1e5 sampled points.  a, b are so large that the 51 x 51 orders
+    land all over the spectrum, on both sides of the evanescent cut."""
+    from closed_forms import grating_field
+    cfg = synth.CONFIGS[name]
+    ny, nx, lam, n, z, pitch = cfg.ny, cfg.nx, cfg.lambdas[0], cfg.n_refr[0], cfg.z, cfg.pitch
+    c = m1 + m2
+    assert c + m1 + m2 <= 2 * np.pi * (n - 1) * cfg.h_max / lam       # 0 <= h <= h_max
+    xs = torch.arange(nx, device=DEV, dtype=torch.int64)
+    sinx = m1 * torch.sin(2 * np.pi * ((a * xs) % nx).double() / nx)
+    h = torch.empty((ny, nx), dtype=torch.float32, device=DEV)
+    rows = max(1, (1 << 26) // nx)
+    for y0 in range(0, ny, rows):
+        ys = torch.arange(y0, min(ny, y0 + rows), device=DEV, dtype=torch.int64)
+        siny = m2 * torch.sin(2 * np.pi * ((b * ys) % ny).double() / ny)
+        h[y0:y0 + rows] = ((c + siny[:, None] + sinx[None, :]) * (lam / (2 * np.pi * (n - 1)))).float()
+    plan = dop.Plan(ny, nx, pitch, (lam,), (n,), z, dop.DOP_LOSS_NONE, 0.0, 0, DEV)
+    inten = torch.empty((1, ny, nx), dtype=torch.float32, device=DEV)
+    plan.fwd(h, None, inten, None)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(17)
+    sy, sx = rng.integers(0, ny, nsamp), rng.integers(0, nx, nsamp)
+    ty, tx = torch.from_numpy(sy).to(DEV), torch.from_numpy(sx).to(DEV)
+    us = plan.field()[0][ty, tx].cpu().numpy().astype(np.complex128)
+    Is = inten[0][ty, tx].cpu().numpy().astype(np.float64)
+    plan.close()
+    ref, Hkl = grating_field(ny, nx, pitch, lam, z, a, b, m1, m2, c, sy, sx)
+    if expect_cut:
+        assert 0.05 < np.mean(Hkl == 0) < 0.95, "orders must fall on both sides of the evanescent cut"
+    e2 = np.linalg.norm(us - ref) / np.linalg.norm(ref)
+    ep = np.abs(us - ref).max() / np.abs(ref).max()
+    assert e2 <= TOL_L2 and ep <= TOL_PEAK, f"{name} grating field: rel-L2 {e2:.3e}, max-abs/peak {ep:.3e}"
+    Ir = np.abs(ref) ** 2
+    e2 = np.linalg.norm(Is - Ir) / np.linalg.norm(Ir)
+    ep = np.abs(Is - Ir).max() / Ir.max()
+    assert e2 <= TOL_L2 and ep <= TOL_PEAK, f"{name} grating intensity: rel-L2 {e2:.3e}, max-abs/peak {ep:.3e}"
+
+
+def test_C2_full_size_phase_grating_closed_form():
+    grating_case("C2", 1511, 977, expect_cut=False)   # (pitch 0.5 um: this grid holds no evanescent bin)
+
+
+@HUGE
+def test_C4_full_size_phase_grating_closed_form():
+    grating_case("C4", 14011, 9007)
+
+
+@HUGE
+def test_C5_full_size_phase_grating_closed_form():
+    grating_case("C5", 14011, 3 * 4001)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_full_size_on_the_bench_inputs_against_the_oracle(name):
+    """Pin P-l ("C1-C3 always"): the bench's own seeded inputs at full size, in the launch
+    configuration bench.py times, element by element against the full-size fp64 oracle: every wavelength
+    for C2, pre-filter on for C3 (about 20 s / 70 s of oracle time on 16 host cores)."""
+    cfg = synth.CONFIGS[name]
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I, L, g = run_l2(cfg, h, T)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, f"{name} intensity")
+    check(g, gr, f"{name} dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
