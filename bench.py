@@ -5,9 +5,12 @@ roofline and the fp64 CPU oracle timed beside it.
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config C1..C5] [--impl reference]
 
 A step = one pass of the whole hot path (dop_propagate_fwd + dop_propagate_adj, every
-wavelength) over one batch of seeded synthetic input.  Default workload: BASELINE.json
-configs[1] (C2: 8192 x 8192, 3 wavelengths).  N > 1 = N independent replicas, one per GPU
-("replicas only"): no data-path collective, weak scaling.
+wavelength) over one batch of seeded synthetic input.  BASELINE.json's metric names no
+configuration and north_star sets its bar "on the largest grid that fits one GPU", so the default
+workload is the largest of C5, C4, C3, C2, C1 whose buffers fit the device's free memory (C5:
+98304 x 65536, 120 GiB on a 180 GB B200); --config selects any other.  N > 1 = N independent
+replicas, one per GPU ("replicas only"): no data-path collective, weak scaling; without
+a torchrun environment --gpus N re-launches itself under torch.distributed.run.
 
 Prints ONE JSON line (rank 0).  `value` = Gpoints/s with inputs resident in HBM; `e2e` = the same
 metric with host buffers (pinned) and host<->device copies inside the timed region; `roofline` =
@@ -129,20 +132,45 @@ def measured_peak_gbs():
 
 
 def ncu_traffic(cfg_name: str, pass_name: str):
-    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant pass from
-    the committed `ncu --set full` capture (profiles/traffic.csv: config,pass,bytes), if any."""
+    """(DRAM bytes per launch, note) of the dominant pass: dram__bytes_read.sum + dram__bytes_write.sum
+    from the committed `ncu --set full` capture of one step (profiles/r02_ncu_<config>.csv, written by
+    paper_2505_22313_b200/ncu_summary.py).  The capture records the hash of the kernel sources it was
+    taken with; a capture of other sources is refused (traffic = null) rather than quoted."""
+    import csv
+    from paper_2505_22313_b200 import build as dop_build
+    path = os.path.join(ROOT, "profiles", f"r02_ncu_{cfg_name}.csv")
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
-            for line in f:
-                if line.startswith("#") or line.count(",") < 2:
-                    continue
-                cfg, rest = line.strip().split(",", 1)      # pass names contain commas:
-                name, nbytes = rest.rsplit(",", 1)           # config , pass ... , bytes
-                if cfg == cfg_name and name == pass_name:
-                    return float(nbytes)
-    except Exception:
-        pass
-    return None
+        with open(path) as f:
+            stamp = f.readline().strip()
+            if not stamp.startswith("# source_stamp="):
+                return None, f"{os.path.basename(path)}: no source stamp"
+            if stamp.split("=", 1)[1] != dop_build.source_stamp():
+                return None, f"{os.path.basename(path)} was captured with other kernel sources (stale): refused"
+            rows = [r for r in csv.DictReader(l for l in f if not l.startswith("#"))]
+        vals = [float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]) for r in rows
+                if r["pass"].split(":", 1)[-1] == pass_name]
+        if vals:
+            return sum(vals) / len(vals), f"{os.path.basename(path)}, {len(vals)} launch(es) of one step"
+        return None, f"{os.path.basename(path)}: pass not in the capture"
+    except FileNotFoundError:
+        return None, "no committed ncu capture for this config"
+    except Exception as e:  # a malformed file must not take the bench down
+        return None, f"{os.path.basename(path)}: {type(e).__name__}"
+
+
+def device_bytes_needed(cfg) -> int:
+    """Device memory of one replica: fields + (pre-filter plane) + h, T, grad (+ I) + slack."""
+    n = cfg.ny * cfg.nx
+    planes = 3 + (len(cfg.lambdas) if cfg.write_intensity else 0) + (1 if cfg.sigma_px > 0 else 0)
+    return n * 8 * len(cfg.lambdas) + n * 4 * planes + (2 << 30)
+
+
+def pick_default_config(free_bytes: int) -> str:
+    from paper_2505_22313_b200 import synth
+    for name in ("C5", "C4", "C3", "C2", "C1"):
+        if device_bytes_needed(synth.CONFIGS[name]) <= free_bytes:
+            return name
+    return "C1"
 
 
 def max_over_ranks(ms: float, dist, device) -> float:
@@ -199,14 +227,36 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--config", default=None, choices=["C1", "C2", "C3", "C4", "C5"],
+                    help="default: the largest configuration that fits the device (C5 on a 180 GB B200)")
     ap.add_argument("--impl", default="dop", choices=["dop", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="do not replay launch-bound configs as a CUDA graph")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    # --gpus N must be what runs: under torchrun WORLD_SIZE has to agree; a bare `bench.py --gpus N`
+    # (N > 1) re-launches itself as N ranks, one per GPU
+    env_world = os.environ.get("WORLD_SIZE")
+    if env_world is None and args.gpus > 1:
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                  f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+                                  "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
+    if env_world is not None and int(env_world) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={env_world}; launch one rank per GPU")
     if args.impl == "reference":
+        if args.config is None:  # a bounded sample of the workload the dop arm picks on this box
+            args.config = "C5"
+            try:
+                import torch
+                if torch.cuda.is_available():
+                    args.config = pick_default_config(torch.cuda.mem_get_info(0)[0])
+            except Exception:
+                pass
         run_reference(args)
         return
 
@@ -220,6 +270,8 @@ def main():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    if args.config is None:
+        args.config = pick_default_config(torch.cuda.mem_get_info(dev)[0])
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -333,9 +385,10 @@ def main():
         p_["share"] = round(acc[key][0] / total_prof, 4)
     dom = max(passes, key=lambda p_: p_["share"])
     step_bytes = sum(acc[k][3] for k in order) / prof_steps * npts_plane
+    traffic, traffic_note = ncu_traffic(args.config, dom["pass"])
     roofline = {
         "bound": "hbm", "kernel": dom["pass"], "achieved": dom["GBps"], "peak": peak, "unit": "GB/s",
-        "frac": round(dom["GBps"] / peak, 4), "traffic": ncu_traffic(args.config, dom["pass"]),
+        "frac": round(dom["GBps"] / peak, 4), "traffic": traffic, "traffic_source": traffic_note,
         "peak_source": peak_src, "bytes_per_launch": dom["bytes_per_point"] * npts_plane,
         "avg_launch_ms": dom["avg_ms"], "share_of_step": dom["share"],
         "whole_step": {"algorithmic_bytes_per_point": step_bytes / points,

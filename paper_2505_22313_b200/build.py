@@ -61,6 +61,15 @@ def _dep_stamp() -> str:
     return h.hexdigest()
 
 
+def source_stamp() -> str:
+    """Hash of the kernel sources only (csrc/ + include/dop.h): what an ncu capture is valid for."""
+    h = hashlib.sha256()
+    for d in sorted(os.listdir(CSRC)) + [os.path.join("..", "..", "include", "dop.h")]:
+        with open(os.path.join(CSRC, d), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def _stale() -> bool:
     stamp = os.path.join(OBJDIR, "stamp")
     if not os.path.exists(LIB) or not os.path.exists(stamp):

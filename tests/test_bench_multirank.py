@@ -55,3 +55,36 @@ def test_reference_arm_runs_on_rank0_only():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_flag_must_agree_with_the_launch():
+    """bench.py --gpus N under a launcher whose WORLD_SIZE differs fails instead of silently running N = 1."""
+    env = dict(os.environ, RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2"], env=env, capture_output=True,
+                       text=True, timeout=120)
+    assert r.returncode != 0 and "WORLD_SIZE=1" in (r.stderr + r.stdout)
+
+
+def test_default_workload_is_the_largest_that_fits():
+    import bench
+    assert bench.pick_default_config(int(178e9)) == "C5"      # 120 GiB + slack on a 180 GB B200
+    assert bench.pick_default_config(int(120e9)) == "C4"      # 96 GiB with the intensity plane
+    assert bench.pick_default_config(int(40e9)) == "C3"
+    assert bench.pick_default_config(int(3e9)) == "C1"
+
+
+def test_stale_ncu_capture_is_refused(tmp_path, monkeypatch):
+    """roofline.traffic comes from a committed capture only if it was taken with the current kernel sources."""
+    import bench
+    from paper_2505_22313_b200 import build as dop_build
+    prof = tmp_path / "profiles"
+    prof.mkdir()
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))
+    body = "pass,kernel,time_us,dram_bytes_read,dram_bytes_write\nfwd:y0:y-fwd,k,1,100,50\nadj:y0:y-fwd,k,1,102,52\n"
+    (prof / "r02_ncu_C9.csv").write_text("# source_stamp=deadbeef\n# note\n" + body)
+    val, note = bench.ncu_traffic("C9", "y0:y-fwd")
+    assert val is None and "stale" in note
+    (prof / "r02_ncu_C9.csv").write_text(f"# source_stamp={dop_build.source_stamp()}\n# note\n" + body)
+    val, note = bench.ncu_traffic("C9", "y0:y-fwd")
+    assert val == 152.0 and "2 launch" in note
+    assert bench.ncu_traffic("C8", "y0:y-fwd")[0] is None
