@@ -67,8 +67,22 @@ typedef enum {
 
 typedef enum {
     DOP_LOSS_NONE = 0, /* fwd writes I (and keeps the field); adj takes the caller's dL/dI       */
-    DOP_LOSS_L2 = 1    /* L = sum_lambda mean_xy (I_lambda - T)^2, seeded inside the pass (Eq. 4) */
+    DOP_LOSS_L2 = 1,   /* L = sum_lambda mean_xy (I_lambda - T)^2, seeded inside the pass (Eq. 4) */
+    DOP_LOSS_SIMSE = 2 /* the paper's penalty, Eq. (6): L = sum_lambda [ L_si-mse +
+                          energy_beta L_energy ].  The paper defers both definitions to a supplement
+                          that is not available; READING: per wavelength
+                          L_si-mse = mean_xy (s I - T)^2 with the least-squares scale s = <I,T>/<I,I>,
+                          L_energy = 1 - mean_xy I.  The scale needs <I,T>, <I,I> of the whole plane
+                          before the seed, so the row pass around the loss splits in two: fwd ends with
+                          "x-inv, store u, plane sums", adj starts with "seed from u, T, s; x-fwd".    */
 } dop_loss_mode;
+
+/* element type of the design layout handed in as d_height (gray-level layouts) */
+typedef enum {
+    DOP_LAYOUT_F32 = 0, /* heights in metres                                                       */
+    DOP_LAYOUT_U8 = 1,  /* gray levels, height = level * layout_step                               */
+    DOP_LAYOUT_U16 = 2  /* gray levels (e.g. the paper's 10-bit layouts), height = level * step    */
+} dop_layout_dtype;
 
 /* flags */
 #define DOP_WRITE_INTENSITY 0x1u /* DOP_LOSS_L2 only: also write I to d_intensity                */
@@ -109,7 +123,26 @@ typedef struct {
     double prefilter_sigma_px; /* 0 = off; > 0 = Gaussian spectral pre-filter on h (config 3)    */
     uint32_t flags;            /* DOP_WRITE_INTENSITY                                            */
     const dop_tuning* tuning;  /* HOST, copied; NULL = defaults                                  */
+    /* ---- the design loop around the path; all zero = the plain path above ---- */
+    double energy_beta;        /* DOP_LOSS_SIMSE: weight of L_energy (paper: 5e-3)                */
+    int32_t upsample;          /* r = 0 | 1 (none), 2, 4, 8: super-resolved design variable       */
+                               /* (PAPER.md:51, 141, 259-264): d_height is the COARSE layout      */
+                               /* [ny/r][nx/r], nearest-neighbour up-sampled r x r inside the     */
+                               /* first pass's read; d_grad_height is [ny/r][nx/r], the r x r     */
+                               /* sum-pool of dL/dh (deterministic: lanes, then rows)             */
+    int32_t layout_dtype;      /* dop_layout_dtype of d_height                                    */
+    double layout_step;        /* metres per gray level (U8 / U16 layouts)                        */
 } dop_plan_desc;
+
+/* Adam with a cosine learning-rate schedule (Kingma & Ba 2014, Algorithm 1), applied
+ * to the design layout as a pointwise epilogue of the adjoint pass. */
+typedef struct {
+    double lr0;          /* initial learning rate, in the unit of the layout (metres)                */
+    double beta1, beta2; /* 0.9, 0.999                                                                */
+    double eps;          /* in the unit of the gradient                                              */
+    int64_t iter;        /* 0-based iteration: lr = lr0 (1 + cos(pi iter/total_iters))/2, t = iter+1 */
+    int64_t total_iters; /* the schedule reaches zero here (paper: 3000)                             */
+} dop_adam;
 
 /*
  * Build a plan (host-only work: validation, factorisation of ny and nx into radix-2/3/4 digit
@@ -125,19 +158,22 @@ dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* works
 /*
  * Forward pass, Eq. (1)-(4): for every lambda  h -> Phi -> u0 = exp(i Phi) -> F -> (x) H ->
  * F^-1 -> I = |u|^2 [-> L2 loss and the seed g_u = 2 (dL/dI) u of the adjoint, DOP_LOSS_L2].
- *   d_height     [ny][nx] fp32 DEVICE, metres, read-only.
- *   d_target     [ny][nx] fp32 DEVICE (shared by all lambda); required for DOP_LOSS_L2,
- *                ignored (may be NULL) for DOP_LOSS_NONE.
+ *   d_height     the design layout, DEVICE, read-only: [ny][nx] fp32 metres, or with upsample = r
+ *                the coarse [ny/r][nx/r] layout of layout_dtype (gray levels times layout_step).
+ *   d_target     [ny][nx] fp32 DEVICE (shared by all lambda); required for DOP_LOSS_L2 and
+ *                DOP_LOSS_SIMSE, ignored (may be NULL) for DOP_LOSS_NONE.  DOP_LOSS_SIMSE: the seed
+ *                is formed from it inside dop_propagate_adj, so the buffer must stay valid and
+ *                unchanged until that call has been enqueued and executed.
  *   d_intensity  [n_lambda][ny][nx] fp32 DEVICE; required for DOP_LOSS_NONE and for
  *                DOP_LOSS_L2 with DOP_WRITE_INTENSITY; otherwise ignored (may be NULL).
- *   d_loss       DEVICE double scalar or NULL; DOP_LOSS_L2: receives L when the stream reaches
- *                that point.  Ignored for DOP_LOSS_NONE.
+ *   d_loss       DEVICE double scalar or NULL; DOP_LOSS_L2 / DOP_LOSS_SIMSE: receives L when the
+ *                stream reaches that point.  Ignored for DOP_LOSS_NONE.
  *   d_workspace  DEVICE, workspace_bytes from dop_plan_create, 256-byte aligned.
  *                After a DOP_LOSS_NONE forward its first n_lambda*ny*nx complex64 (interleaved
  *                re, im) hold the destination field u of Eq. (3), natural order.
  *   cuda_stream  cudaStream_t.
  */
-dop_status dop_propagate_fwd(dop_plan* plan, const float* d_height, const float* d_target,
+dop_status dop_propagate_fwd(dop_plan* plan, const void* d_height, const float* d_target,
                              float* d_intensity, double* d_loss, void* d_workspace,
                              void* cuda_stream);
 
@@ -149,8 +185,24 @@ dop_status dop_propagate_fwd(dop_plan* plan, const float* d_height, const float*
  *                  DOP_LOSS_L2 (the seed was formed inside the forward pass).
  *   d_grad_height  [ny][nx] fp32 DEVICE, overwritten with dL/dh.
  */
-dop_status dop_propagate_adj(dop_plan* plan, const float* d_height, const float* d_dLdI,
+dop_status dop_propagate_adj(dop_plan* plan, const void* d_height, const float* d_dLdI,
                              float* d_grad_height, void* d_workspace, void* cuda_stream);
+
+/*
+ * The adjoint pass with the Adam update of the design layout fused into its last store (no up-sampling,
+ * no pre-filter: the A5 store of the last wavelength) or into the final row-pooling kernel (up-sampling),
+ * else run as one pointwise kernel after the pre-filter adjoint.
+ *   d_layout       the fp32 design layout (DOP_LAYOUT_F32 only), the buffer that was given to
+ *                  dop_propagate_fwd; UPDATED IN PLACE: l <- l - lr m_hat / (sqrt(v_hat) + eps).
+ *   d_grad_height  dL/dl, same shape as the layout; may be NULL when only the update is wanted.
+ *   d_m, d_v       Adam's first / second moment, fp32, same shape as the layout, caller-owned,
+ *                  zero before the first iteration; updated in place.
+ *   hp             HOST, read during the call.
+ * Errors as dop_propagate_adj; DOP_ERR_INVALID_ARG for a non-fp32 layout or bad hyper-parameters.
+ */
+dop_status dop_propagate_adj_adam(dop_plan* plan, float* d_layout, const float* d_dLdI, float* d_grad_height,
+                                  float* d_m, float* d_v, const dop_adam* hp, void* d_workspace,
+                                  void* cuda_stream);
 
 /* Frees the plan's host memory and device tables.  NULL -> DOP_ERR_INVALID_ARG. */
 dop_status dop_plan_destroy(dop_plan* plan);

@@ -31,13 +31,21 @@ namespace {
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Buffers {
-    const float* height = nullptr; // what LD_HEIGHT / ST_GRAD read (h or h_eff)
+    const void* height = nullptr;  // what LD_HEIGHT / ST_GRAD read: the caller's layout, or the fine fp32 h_eff plane
+    bool height_is_layout = false; // -> plan's up-sampling factor and layout dtype apply to `height`
     const float* target = nullptr;
     float* intensity = nullptr;
     const float* dLdI = nullptr;
-    float* grad = nullptr;
-    const float* real_src = nullptr;
+    float* grad = nullptr;         // where ST_GRAD writes: a fine plane, or (grad_pool) the x-pooled plane
+    bool grad_pool = false;
+    const void* real_src = nullptr;
+    bool real_src_is_layout = false;
     float* real_dst = nullptr;
+    bool real_dst_pool = false;
+    const AdamParams* adam = nullptr; // fused into the ST_GRAD store of the last wavelength
+    float* adam_m = nullptr;
+    float* adam_v = nullptr;
+    float* adam_h = nullptr;
 };
 
 dop_status ensure_device(dop_plan* p)
@@ -129,10 +137,34 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.mid_op = t.mid_op;
     d.store_op = t.store_op;
     d.field = (float2*)(ws + align256(npts * sizeof(float2)) * (size_t)lam);
-    d.height = b.height;
+    d.height = (const float*)b.height;
     d.write_intensity = 0;
+    d.cnx = p->desc.nx >> p->up_lg;
+    d.lpr = (d.col_type || d.cluster) ? 0 : p->desc.nx / d.L;
+    d.h_step = (float)p->desc.layout_step;
+    const bool hl = (t.load_op == LD_HEIGHT || t.store_op == ST_GRAD) && b.height_is_layout;
+    if (hl) { d.up_lg = p->up_lg; d.h_dtype = (int)p->desc.layout_dtype; }
     if (t.load_op == LD_SEED) d.plane_in = b.dLdI + npts * (size_t)lam;
-    if (t.load_op == LD_REAL) d.plane_in = b.real_src;
+    if (t.load_op == LD_SEED_SIMSE) {
+        d.plane_in = b.target;
+        d.coef = (const float*)(ws + p->ws_coef_off) + 4 * (size_t)lam;
+    }
+    if (t.load_op == LD_REAL) {
+        d.plane_in = (const float*)b.real_src;
+        if (b.real_src_is_layout && (p->up_lg > 0 || p->desc.layout_dtype != DOP_LAYOUT_F32)) {
+            d.coarse_in = 1;
+            d.up_lg = p->up_lg;
+            d.h_dtype = (int)p->desc.layout_dtype;
+        }
+    }
+    if (t.store_op == ST_C64_STATS) {
+        d.plane_in = b.target;
+        d.loss_scratch = (double*)(ws + p->ws_loss_off) + 4 * (size_t)p->loss_tiles * (size_t)lam;
+        if (p->desc.flags & DOP_WRITE_INTENSITY) {
+            d.write_intensity = 1;
+            d.plane_out = b.intensity + npts * (size_t)lam;
+        }
+    }
     if (t.mid_op == MID_LOSS) {
         d.plane_in = b.target;
         d.loss_scratch = (double*)(ws + p->ws_loss_off) + (size_t)p->loss_tiles * (size_t)lam;
@@ -144,9 +176,19 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     if (t.store_op == ST_GRAD) {
         d.plane_out = b.grad;
         if (lam > 0) d.store_op = ST_GRAD_ACC;
+        if (b.grad_pool) { d.pool_out = 1; d.up_lg = p->up_lg; }
+        if (b.adam != nullptr && lam == p->desc.n_lambda - 1) {
+            d.adam_m = b.adam_m; d.adam_v = b.adam_v; d.adam_h = b.adam_h;
+            d.adam_b1 = b.adam->b1; d.adam_b2 = b.adam->b2; d.adam_c1 = b.adam->c1; d.adam_c2 = b.adam->c2;
+            d.adam_a1 = b.adam->a1; d.adam_rb2 = b.adam->rb2;
+            d.adam_eps = b.adam->eps;
+        }
     }
     if (t.store_op == ST_C64_INTENSITY) d.plane_out = b.intensity + npts * (size_t)lam;
-    if (t.store_op == ST_REAL) d.plane_out = b.real_dst;
+    if (t.store_op == ST_REAL) {
+        d.plane_out = b.real_dst;
+        if (b.real_dst_pool) { d.pool_out = 1; d.up_lg = p->up_lg; }
+    }
     const double lambda = p->lambda[(size_t)lam], n = p->n_refr[(size_t)lam];
     d.phase_coef = (float)((n - 1.0) / lambda);
     d.grad_coef = (float)(2.0 * M_PI * (n - 1.0) / lambda);
@@ -330,7 +372,7 @@ dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* works
     if (d->n_lambda < 1 || d->n_lambda > 4096) return DOP_ERR_INVALID_ARG;
     if (!(d->pitch > 0.0) || !std::isfinite(d->pitch) || !std::isfinite(d->z)) return DOP_ERR_INVALID_ARG;
     if (!(d->prefilter_sigma_px >= 0.0) || !std::isfinite(d->prefilter_sigma_px)) return DOP_ERR_INVALID_ARG;
-    if (d->loss != DOP_LOSS_NONE && d->loss != DOP_LOSS_L2) return DOP_ERR_INVALID_ARG;
+    if (d->loss != DOP_LOSS_NONE && d->loss != DOP_LOSS_L2 && d->loss != DOP_LOSS_SIMSE) return DOP_ERR_INVALID_ARG;
     if (d->flags & ~DOP_WRITE_INTENSITY) return DOP_ERR_INVALID_ARG;
     for (int i = 0; i < d->n_lambda; ++i) {
         if (!(d->lambda[i] > 0.0) || !std::isfinite(d->lambda[i])) return DOP_ERR_INVALID_ARG;
@@ -358,40 +400,51 @@ dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* works
     return DOP_OK;
 }
 
-dop_status dop_propagate_fwd(dop_plan* p, const float* d_height, const float* d_target, float* d_intensity,
+dop_status dop_propagate_fwd(dop_plan* p, const void* d_height, const float* d_target, float* d_intensity,
                              double* d_loss, void* d_workspace, void* cuda_stream)
 {
     if (p == nullptr || d_height == nullptr) return DOP_ERR_INVALID_ARG;
-    const bool l2 = p->desc.loss == DOP_LOSS_L2;
-    const bool need_I = !l2 || (p->desc.flags & DOP_WRITE_INTENSITY);
-    if (l2 && d_target == nullptr) return DOP_ERR_INVALID_ARG;
+    const bool l2 = p->desc.loss == DOP_LOSS_L2, simse = p->desc.loss == DOP_LOSS_SIMSE;
+    const bool need_I = !(l2 || simse) || (p->desc.flags & DOP_WRITE_INTENSITY);
+    if ((l2 || simse) && d_target == nullptr) return DOP_ERR_INVALID_ARG;
     if (need_I && d_intensity == nullptr) return DOP_ERR_INVALID_ARG;
     if (d_workspace == nullptr) return DOP_ERR_WORKSPACE;
     dop_status s = ensure_device(p);
     if (s != DOP_OK) return s;
     p->state = 0;
     p->prof_n = 0;
+    p->target_seen = d_target;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
     Buffers b;
     b.height = d_height;
+    b.height_is_layout = true;
     b.target = d_target;
     b.intensity = d_intensity;
-    if (!p->pre.empty()) { // F0: h_eff = Re F^-1{ F{h} G }
+    if (!p->pre.empty()) { // F0: h_eff = Re F^-1{ F{U l} G } (the layout is up-sampled inside the first read)
         float* heff = (float*)(ws + p->ws_heff_off);
         Buffers pb;
         pb.real_src = d_height;
+        pb.real_src_is_layout = true;
         pb.real_dst = heff;
         if ((s = run(p, p->pre, 0, pb, ws, st, "pre")) != DOP_OK) return s;
         b.height = heff;
+        b.height_is_layout = false;
     }
     for (int lam = 0; lam < p->desc.n_lambda; ++lam)
         if ((s = run(p, p->fwd, lam, b, ws, st, "fwd")) != DOP_OK) return s;
+    const double npts = (double)p->desc.nx * (double)p->desc.ny;
     if (l2 && d_loss != nullptr) {
-        const double inv_n = 1.0 / ((double)p->desc.nx * (double)p->desc.ny);
         long long slot = prof_begin(p, "fwd:loss-reduce", 0.0, st);
         cudaError_t e = launch_loss_reduce((const double*)(ws + p->ws_loss_off), p->loss_tiles * p->desc.n_lambda,
-                                           inv_n, d_loss, st);
+                                           1.0 / npts, d_loss, st);
+        prof_end(p, slot, st);
+        if (e != cudaSuccess) return DOP_ERR_CUDA;
+    }
+    if (simse) { // plane sums -> s, L, seed coefficients (needed by adj even when the caller does not want L)
+        long long slot = prof_begin(p, "fwd:si-mse-reduce", 0.0, st);
+        cudaError_t e = launch_simse_reduce((const double*)(ws + p->ws_loss_off), p->loss_tiles, p->desc.n_lambda, npts,
+                                            p->desc.energy_beta, (float*)(ws + p->ws_coef_off), d_loss, st);
         prof_end(p, slot, st);
         if (e != cudaSuccess) return DOP_ERR_CUDA;
     }
@@ -399,31 +452,94 @@ dop_status dop_propagate_fwd(dop_plan* p, const float* d_height, const float* d_
     return DOP_OK;
 }
 
-dop_status dop_propagate_adj(dop_plan* p, const float* d_height, const float* d_dLdI, float* d_grad_height,
-                             void* d_workspace, void* cuda_stream)
+static dop_status propagate_adj(dop_plan* p, const void* d_height, const float* d_dLdI, float* d_grad_height,
+                                void* d_workspace, void* cuda_stream, const dop_adam* hp, float* d_m, float* d_v)
 {
     if (p == nullptr || d_height == nullptr || d_grad_height == nullptr) return DOP_ERR_INVALID_ARG;
     if (p->desc.loss == DOP_LOSS_NONE && d_dLdI == nullptr) return DOP_ERR_INVALID_ARG;
     if (d_workspace == nullptr) return DOP_ERR_WORKSPACE;
+    AdamParams ap{};
+    if (hp != nullptr) {
+        if (d_m == nullptr || d_v == nullptr || p->desc.layout_dtype != DOP_LAYOUT_F32) return DOP_ERR_INVALID_ARG;
+        if (!(hp->lr0 >= 0.0) || !(hp->beta1 >= 0.0 && hp->beta1 < 1.0) || !(hp->beta2 >= 0.0 && hp->beta2 < 1.0) ||
+            !(hp->eps >= 0.0) || hp->iter < 0 || hp->total_iters < 1 || !std::isfinite(hp->lr0) || !std::isfinite(hp->eps))
+            return DOP_ERR_INVALID_ARG;
+        const double t = (double)hp->iter + 1.0;
+        const double frac = (double)(hp->iter < hp->total_iters ? hp->iter : hp->total_iters) / (double)hp->total_iters;
+        const double lr = hp->lr0 * 0.5 * (1.0 + std::cos(M_PI * frac));
+        ap.b1 = (float)hp->beta1;
+        ap.b2 = (float)hp->beta2;
+        ap.c1 = (float)(1.0 - hp->beta1);
+        ap.c2 = (float)(1.0 - hp->beta2);
+        ap.a1 = (float)(lr / (1.0 - std::pow(hp->beta1, t)));
+        ap.rb2 = (float)(1.0 / (1.0 - std::pow(hp->beta2, t)));
+        ap.eps = (float)hp->eps;
+    }
     if (p->state != 1) return DOP_ERR_STATE;
     dop_status s = ensure_device(p);
     if (s != DOP_OK) return s;
     p->state = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
+    const bool has_pre = !p->pre.empty();
+    const bool pooled = p->up_lg > 0;
+    const bool plain_layout = !pooled && p->desc.layout_dtype == DOP_LAYOUT_F32;
+    float* xpool = (float*)(ws + p->ws_xpool_off);
     Buffers b;
-    b.height = p->pre.empty() ? d_height : (const float*)(ws + p->ws_heff_off);
     b.dLdI = d_dLdI;
-    b.grad = d_grad_height;
+    b.target = nullptr;
+    if (has_pre) {
+        b.height = ws + p->ws_heff_off; // the filtered fine plane
+        b.grad = plain_layout ? d_grad_height : (float*)(ws + p->ws_gfine_off);
+    } else {
+        b.height = d_height;
+        b.height_is_layout = true;
+        b.grad = pooled ? xpool : d_grad_height;
+        b.grad_pool = pooled;
+        if (hp != nullptr && !pooled) { // Adam rides on the A5 store of the last wavelength
+            b.adam = &ap;
+            b.adam_m = d_m;
+            b.adam_v = d_v;
+            b.adam_h = (float*)const_cast<void*>(d_height);
+        }
+    }
+    if (p->desc.loss == DOP_LOSS_SIMSE) b.target = p->target_seen;
     for (int lam = 0; lam < p->desc.n_lambda; ++lam)
         if ((s = run(p, p->adj, lam, b, ws, st, "adj")) != DOP_OK) return s;
-    if (!p->pre.empty()) { // A6: the Gaussian spectrum is real and even, so the filter is self-adjoint
+    if (has_pre) { // A6: the Gaussian spectrum is real and even, so the filter is self-adjoint
         Buffers pb;
-        pb.real_src = d_grad_height;
-        pb.real_dst = d_grad_height;
+        pb.real_src = b.grad;
+        pb.real_dst = pooled ? xpool : d_grad_height;
+        pb.real_dst_pool = pooled;
         if ((s = run(p, p->pre, 0, pb, ws, st, "pre-adj")) != DOP_OK) return s;
     }
+    const long long cny = p->desc.ny >> p->up_lg, cnx = p->desc.nx >> p->up_lg;
+    if (pooled) { // rows of the x-pooled plane -> coarse dL/dl (+ Adam on the coarse layout)
+        long long slot = prof_begin(p, "adj:pool-rows", 4.0 / (double)(1 << p->up_lg), st);
+        cudaError_t e = launch_pool_rows(xpool, d_grad_height, cny, cnx, 1 << p->up_lg, hp != nullptr ? &ap : nullptr,
+                                         (float*)const_cast<void*>(d_height), d_m, d_v, st);
+        prof_end(p, slot, st);
+        if (e != cudaSuccess) return DOP_ERR_CUDA;
+    } else if (hp != nullptr && has_pre) {
+        long long slot = prof_begin(p, "adj:adam", 28.0, st);
+        cudaError_t e = launch_adam(d_grad_height, cny * cnx, ap, (float*)const_cast<void*>(d_height), d_m, d_v, st);
+        prof_end(p, slot, st);
+        if (e != cudaSuccess) return DOP_ERR_CUDA;
+    }
     return DOP_OK;
+}
+
+dop_status dop_propagate_adj(dop_plan* p, const void* d_height, const float* d_dLdI, float* d_grad_height,
+                             void* d_workspace, void* cuda_stream)
+{
+    return propagate_adj(p, d_height, d_dLdI, d_grad_height, d_workspace, cuda_stream, nullptr, nullptr, nullptr);
+}
+
+dop_status dop_propagate_adj_adam(dop_plan* p, float* d_layout, const float* d_dLdI, float* d_grad_height, float* d_m,
+                                  float* d_v, const dop_adam* hp, void* d_workspace, void* cuda_stream)
+{
+    if (hp == nullptr) return DOP_ERR_INVALID_ARG;
+    return propagate_adj(p, d_layout, d_dLdI, d_grad_height, d_workspace, cuda_stream, hp, d_m, d_v);
 }
 
 dop_status dop_plan_destroy(dop_plan* p)
@@ -486,7 +602,8 @@ int64_t dop_plan_launch_count(const dop_plan* p)
         return n;
     };
     int64_t n = (count(p->fwd) + count(p->adj)) * p->desc.n_lambda + 2 * count(p->pre);
-    if (p->desc.loss == DOP_LOSS_L2) n += 1;
+    if (p->desc.loss == DOP_LOSS_L2 || p->desc.loss == DOP_LOSS_SIMSE) n += 1; // loss / plane-sum reduction
+    if (p->up_lg > 0) n += 1;                                                  // row pooling
     return n;
 }
 

@@ -96,6 +96,7 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
     const unsigned sbase = cl_smem_u32(s);
 
     float2 v[P];
+    const bool lay = (p.up_lg | p.h_dtype | p.coarse_in | p.pool_out) != 0; // design-layout addressing (uniform)
 
     // ---- staged contiguous line access (last-group layout: thread owns slots 16 tt .. 16 tt + 15, a
     //      warp 512 adjacent slots = 4 KiB; pow2_impl.cuh "STAGE")
@@ -159,6 +160,16 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
     // =========================================================================================
     if (DIR1 > 0) {
         // ---- natural-layout load (+ prologue op)
+        if ((V == V_HEIGHT && lay) || (V == V_LDOTHER && p.coarse_in)) {
+            // design layout: nearest up-sampling / gray levels inside the read (apart from the plain loop below)
+#pragma unroll
+            for (int c = 0; c < P; ++c) {
+                const float hv = ld_layout(V == V_HEIGHT ? (const void*)p.height : (const void*)p.plane_in, p.h_dtype, p.h_step,
+                                           p.up_lg, p.cnx, row, n2 + c * M);
+                if (V == V_HEIGHT) sincos_turns(hv * p.phase_coef, &v[c].y, &v[c].x);
+                else v[c] = make_float2(hv, 0.0f);
+            }
+        } else {
 #pragma unroll
         for (int c = 0; c < P; ++c) {
             const long long off = nat0 + (long long)c * M;
@@ -170,12 +181,18 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
                     const float2 u = p.field[off];
                     const float g = 2.0f * __ldg(p.plane_in + off);
                     v[c] = make_float2(g * u.x, g * u.y);
+                } else if (p.load_op == LD_SEED_SIMSE) {               // Eq. (6): 2 dL/dI = c0 + cI I + cT T
+                    const float2 u = p.field[off];
+                    const float I = u.x * u.x + u.y * u.y;
+                    const float g = fmaf(__ldg(p.coef + 1), I, fmaf(__ldg(p.coef + 2), __ldg(p.plane_in + off), __ldg(p.coef)));
+                    v[c] = make_float2(g * u.x, g * u.y);
                 } else {
                     v[c] = make_float2(__ldg(p.plane_in + off), 0.0f);
                 }
             } else {
                 v[c] = p.field[off];
             }
+        }
         }
     } else {
         load_lines();
@@ -244,6 +261,39 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
         store_lines();
     } else {
         // ---- natural-layout store (+ epilogue op)
+        double st0 = 0.0, st1 = 0.0, st2 = 0.0, st3 = 0.0; // ST_C64_STATS: <I,T>, <I,I>, sum I, <T,T>
+        if ((V == V_GRAD && (lay || p.adam_m != nullptr)) || (V == V_STOTHER && p.pool_out)) {
+            // design-loop flavours of the two real-plane stores (apart from the plain loop below)
+            const bool leader = (tid & ((1 << p.up_lg) - 1)) == 0;
+#pragma unroll
+            for (int c = 0; c < P; ++c) {
+                const long long off = nat0 + (long long)c * M;
+                if (V == V_GRAD) {
+                    const float hv = lay ? ld_layout(p.height, p.h_dtype, p.h_step, p.up_lg, p.cnx, row, n2 + c * M)
+                                         : __ldg(p.height + off);
+                    float sn, cs;
+                    sincos_turns(hv * p.phase_coef, &sn, &cs);
+                    float g = p.grad_coef * (cs * v[c].y - sn * v[c].x); // A5: c Im(conj(u0) g)
+                    if (p.pool_out) {
+                        g = pool_lanes(g, p.up_lg, 0xffffffffu);
+                        const long long ci = row * p.cnx + ((n2 + c * M) >> p.up_lg);
+                        if (leader) {
+                            if (p.store_op == ST_GRAD_ACC) g += p.plane_out[ci];
+                            p.plane_out[ci] = g;
+                        }
+                    } else {
+                        if (p.store_op == ST_GRAD_ACC) g += __ldg(p.plane_out + off);
+                        p.plane_out[off] = g;
+                        if (p.adam_m != nullptr)
+                            p.adam_h[off] = adam_update(g, hv, p.adam_m + off, p.adam_v + off, p.adam_b1, p.adam_b2, p.adam_c1,
+                                                        p.adam_c2, p.adam_a1, p.adam_rb2, p.adam_eps);
+                    }
+                } else {
+                    const float g = pool_lanes(v[c].x, p.up_lg, 0xffffffffu);
+                    if (leader) p.plane_out[row * p.cnx + ((n2 + c * M) >> p.up_lg)] = g;
+                }
+            }
+        } else {
 #pragma unroll
         for (int c = 0; c < P; ++c) {
             const long long off = nat0 + (long long)c * M;
@@ -258,11 +308,42 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
                 if (p.store_op == ST_C64_INTENSITY) {
                     p.field[off] = v[c];
                     p.plane_out[off] = v[c].x * v[c].x + v[c].y * v[c].y;
+                } else if (p.store_op == ST_C64_STATS) {
+                    p.field[off] = v[c];
+                    const float I = v[c].x * v[c].x + v[c].y * v[c].y;
+                    const float Tv = __ldg(p.plane_in + off);
+                    st0 += (double)I * (double)Tv;
+                    st1 += (double)I * (double)I;
+                    st2 += (double)I;
+                    st3 += (double)Tv * (double)Tv;
+                    if (p.write_intensity) p.plane_out[off] = I;
                 } else {
                     p.plane_out[off] = v[c].x;
                 }
             } else {
                 p.field[off] = v[c];
+            }
+        }
+        }
+        if (V == V_STOTHER) {
+            if (p.store_op == ST_C64_STATS) {
+                __shared__ double sred[4][kClThreads / 32];
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) {
+                    st0 += __shfl_down_sync(0xffffffffu, st0, d);
+                    st1 += __shfl_down_sync(0xffffffffu, st1, d);
+                    st2 += __shfl_down_sync(0xffffffffu, st2, d);
+                    st3 += __shfl_down_sync(0xffffffffu, st3, d);
+                }
+                if (lane == 0) {
+                    sred[0][tid >> 5] = st0; sred[1][tid >> 5] = st1; sred[2][tid >> 5] = st2; sred[3][tid >> 5] = st3;
+                }
+                __syncthreads();
+                if (tid < 4) {
+                    double r = 0.0;
+                    for (int w = 0; w < kClThreads / 32; ++w) r += sred[tid][w];
+                    p.loss_scratch[4 * (p.tile0 + blockIdx.x) + tid] = r;
+                }
             }
         }
     }

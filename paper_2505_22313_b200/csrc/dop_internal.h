@@ -28,7 +28,8 @@ enum LoadOp : int {
     LD_C64 = 0,     // complex64 field
     LD_HEIGHT = 1,  // Eq. (1)+(2): u0 = exp(i 2 pi (n-1) h / lambda) from the fp32 height plane
     LD_SEED = 2,    // A1 (DOP_LOSS_NONE): g_u = 2 (dL/dI) u
-    LD_REAL = 3     // pre-filter: fp32 plane -> (v, 0)
+    LD_REAL = 3,    // pre-filter: fp32 plane -> (v, 0)
+    LD_SEED_SIMSE = 4 // A1 (DOP_LOSS_SIMSE): g_u = (c0 + cI |u|^2 + cT T) u, coefficients from the plane sums
 };
 enum MidOp : int {
     MID_NONE = 0,
@@ -42,7 +43,8 @@ enum StoreOp : int {
     ST_GRAD = 1,           // A5: dL/dh  = c Im(conj(u0) g)   (overwrite)
     ST_GRAD_ACC = 2,       //     dL/dh += ...                (lambda > 0)
     ST_C64_INTENSITY = 3,  // DOP_LOSS_NONE forward end: keep u, write I
-    ST_REAL = 4            // pre-filter: Re(v) -> fp32 plane
+    ST_REAL = 4,           // pre-filter: Re(v) -> fp32 plane
+    ST_C64_STATS = 5       // DOP_LOSS_SIMSE forward end: keep u, [write I], plane sums <I,T>, <I,I>, sum I, <T,T>
 };
 
 constexpr int kMaxRadixSteps = 16;
@@ -81,7 +83,22 @@ struct PassDesc {
     const float* height;  // LD_HEIGHT / ST_GRAD*
     const float* plane_in; // LD_SEED: dL/dI;  LD_REAL: source;  MID_LOSS: target T
     float* plane_out;     // ST_GRAD*: grad;  ST_REAL: destination;  *_INTENSITY: I
-    double* loss_scratch; // MID_LOSS: one partial per CTA
+    double* loss_scratch; // MID_LOSS: one partial per CTA;  ST_C64_STATS: four per CTA
+    const float* coef;    // LD_SEED_SIMSE: (c0, cI, cT) of this wavelength
+    // ---- design layout (dop_plan_desc.upsample / layout_dtype): where LD_HEIGHT / ST_GRAD* / LD_REAL (pre-filter
+    //      input) find the height of fine-grid point (row, x), and where ST_GRAD* / ST_REAL (pre-filter adjoint) pool
+    int up_lg;            // log2 of the up-sampling factor r (0 = none)
+    int h_dtype;          // dop_layout_dtype of `height` (LD_HEIGHT, ST_GRAD*) / of plane_in (LD_REAL with coarse_in)
+    float h_step;         // metres per level
+    long long cnx;        // nx / r: row length of the coarse layout and of the x-pooled plane
+    long long lpr;        // row-type tiles: lines per row (nx / L)
+    int coarse_in;        // LD_REAL reads the coarse layout (up-sampled on the fly)
+    int pool_out;         // ST_GRAD* / ST_REAL write the x-pooled plane [ny][nx / r] (sum over r adjacent lanes)
+    // ---- Adam epilogue fused into the A5 store (ST_GRAD* with adam_m != nullptr; no up-sampling)
+    float* adam_m;
+    float* adam_v;
+    float* adam_h;        // the fp32 layout, updated in place
+    float adam_b1, adam_b2, adam_c1, adam_c2, adam_a1, adam_rb2, adam_eps; // c = 1 - b; a1 = lr_t / (1 - b1^t), rb2 = 1 / (1 - b2^t)
     float phase_coef;     // (n-1)/lambda   [turns per metre]
     float grad_coef;      // 2 pi (n-1)/lambda
     float scale;          // 1/(ny nx)
@@ -109,6 +126,16 @@ int pow2_lines(long long L, bool col_type, bool plain = false, int nb_override =
 std::vector<float2> pow2_group_twiddles(long long L);
 cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
                                cudaStream_t stream);
+// DOP_LOSS_SIMSE: plane sums -> scale s, loss, seed coefficients per wavelength (kernels_generic.cu)
+cudaError_t launch_simse_reduce(const double* scratch, long long tiles, int n_lambda, double npts, double beta,
+                                float* coef, double* d_loss, cudaStream_t stream);
+struct AdamParams { float b1, b2, c1, c2, a1, rb2, eps; }; // c1 = 1 - b1, c2 = 1 - b2 (rounded from fp64)
+// rows of the x-pooled plane -> coarse gradient [ny/r][cnx] (+ optional Adam update of the fp32 layout)
+cudaError_t launch_pool_rows(const float* xpool, float* grad, long long cny, long long cnx, int r, const AdamParams* adam,
+                             float* layout, float* m, float* v, cudaStream_t stream);
+// pointwise Adam on a finished gradient plane (pre-filter configurations)
+cudaError_t launch_adam(const float* grad, long long n, const AdamParams& adam, float* layout, float* m, float* v,
+                        cudaStream_t stream);
 
 // ------------------------------------------------------------------------------------------
 // host-side plan
@@ -171,7 +198,8 @@ struct dop_plan {
     // schedules for one lambda
     std::vector<dop::PassTmpl> fwd, adj, pre; // pre = Gaussian pre-filter (real -> real)
     long long loss_tiles = 0;                 // CTAs of the MID_LOSS pass
-    size_t ws_fields = 0, ws_heff_off = 0, ws_loss_off = 0, ws_bytes = 0;
+    size_t ws_fields = 0, ws_heff_off = 0, ws_loss_off = 0, ws_xpool_off = 0, ws_coef_off = 0, ws_gfine_off = 0, ws_bytes = 0;
+    int up_lg = 0;              // log2(upsample)
     // device tables (lazy)
     bool dev_ready = false;
     int device = -1;
@@ -182,6 +210,7 @@ struct dop_plan {
     float* d_g[2] = {nullptr, nullptr};
     std::vector<size_t> pi_off[2];
     int state = 0; // 1 after a successful fwd
+    const float* target_seen = nullptr; // DOP_LOSS_SIMSE: the target of the last fwd (adj forms the seed from it)
     // slab schedule: auxiliary streams the slabs of a segment are dealt to, so that the launch tails of
     // one slab overlap the next slab's kernels (fork / join around the segment on the caller's stream)
     int n_aux = 0;

@@ -107,11 +107,25 @@ __device__ void tile_fft(float2* s, const PassDesc& p, int nl_eff, int sl, int s
     }
 }
 
+// height of the fine-grid point at linear offset `off` from the design layout (nearest up-sampling, gray levels)
+__device__ __forceinline__ float layout_height(const PassDesc& p, const void* base, long long off)
+{
+    if ((p.up_lg | p.h_dtype) == 0) return ((const float*)base)[off];
+    const long long nx = p.cnx << p.up_lg;
+    const long long row = off / nx, x = off - row * nx;
+    const long long ci = (row >> p.up_lg) * p.cnx + (x >> p.up_lg);
+    if (p.h_dtype == DOP_LAYOUT_F32) return ((const float*)base)[ci];
+    if (p.h_dtype == DOP_LAYOUT_U8) return p.h_step * (float)((const unsigned char*)base)[ci];
+    return p.h_step * (float)((const unsigned short*)base)[ci];
+}
+
 template <bool COL>
 __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
 {
     extern __shared__ float2 s[];
     __shared__ double red[8];
+    __shared__ double sred[4][8];
+    double st0 = 0.0, st1 = 0.0, st2 = 0.0, st3 = 0.0; // ST_C64_STATS: <I,T>, <I,I>, sum I, <T,T>
 
     // ---- which tile
     long long t = blockIdx.x;
@@ -139,14 +153,18 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
         if (p.load_op == LD_C64) {
             v = p.field[off];
         } else if (p.load_op == LD_HEIGHT) {
-            float tt = p.height[off] * p.phase_coef; // Eq. (1) in turns
+            float tt = layout_height(p, p.height, off) * p.phase_coef; // Eq. (1) in turns
             sincospif(2.0f * tt, &v.y, &v.x);        // Eq. (2), E_in = 1
         } else if (p.load_op == LD_SEED) {
             float2 u = p.field[off];
             float g = 2.0f * p.plane_in[off];
             v = make_float2(g * u.x, g * u.y);
+        } else if (p.load_op == LD_SEED_SIMSE) {     // Eq. (6): 2 dL/dI = c0 + cI I + cT T
+            float2 u = p.field[off];
+            float g = p.coef[0] + p.coef[1] * (u.x * u.x + u.y * u.y) + p.coef[2] * p.plane_in[off];
+            v = make_float2(g * u.x, g * u.y);
         } else {
-            v = make_float2(p.plane_in[off], 0.0f);
+            v = make_float2(p.coarse_in ? layout_height(p, p.plane_in, off) : p.plane_in[off], 0.0f);
         }
         if (p.tw_b != nullptr && p.fft1_dir < 0) {
             long long r = r0 + (long long)l * r_per_line;
@@ -234,17 +252,51 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
         if (p.store_op == ST_C64) {
             p.field[off] = v;
         } else if (p.store_op == ST_GRAD || p.store_op == ST_GRAD_ACC) {
-            float tt = p.height[off] * p.phase_coef;
+            const float hv = layout_height(p, p.height, off);
+            float tt = hv * p.phase_coef;
             float sn, cs;
             sincospif(2.0f * tt, &sn, &cs); // u0 recomputed, not stored
             float g = p.grad_coef * (cs * v.y - sn * v.x); // A5: c Im(conj(u0) g)
             if (p.store_op == ST_GRAD_ACC) g += p.plane_out[off];
             p.plane_out[off] = g;
+            if (p.adam_m != nullptr) { // Adam (Kingma & Ba 2014, Alg. 1) on the last wavelength's store
+                const float mn = p.adam_b1 * p.adam_m[off] + p.adam_c1 * g;
+                const float vn = p.adam_b2 * p.adam_v[off] + p.adam_c2 * g * g;
+                p.adam_m[off] = mn;
+                p.adam_v[off] = vn;
+                p.adam_h[off] = hv - p.adam_a1 * mn / (sqrtf(vn * p.adam_rb2) + p.adam_eps);
+            }
         } else if (p.store_op == ST_C64_INTENSITY) {
             p.field[off] = v;
             p.plane_out[off] = v.x * v.x + v.y * v.y;
+        } else if (p.store_op == ST_C64_STATS) {
+            p.field[off] = v;
+            const float I = v.x * v.x + v.y * v.y, Tv = p.plane_in[off];
+            st0 += (double)I * (double)Tv;
+            st1 += (double)I * (double)I;
+            st2 += (double)I;
+            st3 += (double)Tv * (double)Tv;
+            if (p.write_intensity) p.plane_out[off] = I;
         } else {
             p.plane_out[off] = v.x;
+        }
+    }
+    if (p.store_op == ST_C64_STATS) {
+        for (int d = 16; d > 0; d >>= 1) {
+            st0 += __shfl_down_sync(0xffffffffu, st0, d);
+            st1 += __shfl_down_sync(0xffffffffu, st1, d);
+            st2 += __shfl_down_sync(0xffffffffu, st2, d);
+            st3 += __shfl_down_sync(0xffffffffu, st3, d);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            const int w = threadIdx.x >> 5;
+            sred[0][w] = st0; sred[1][w] = st1; sred[2][w] = st2; sred[3][w] = st3;
+        }
+        __syncthreads();
+        if (threadIdx.x < 4) {
+            double r = 0.0;
+            for (int w = 0; w < (int)(blockDim.x >> 5); ++w) r += sred[threadIdx.x][w];
+            p.loss_scratch[4 * (p.tile0 + blockIdx.x) + threadIdx.x] = r;
         }
     }
 }
@@ -290,6 +342,103 @@ cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n,
                                cudaStream_t stream)
 {
     loss_reduce_kernel<<<1, 1024, 0, stream>>>(scratch, n, inv_n, d_loss);
+    return cudaGetLastError();
+}
+
+// Eq. (6) (reading in dop.h): fixed-order reduction of the four plane sums of every wavelength,
+// then s = <I,T>/<I,I>, L = sum_lambda [ (<T,T> - <I,T>^2/<I,I>)/N + beta (1 - sum I / N) ] and the coefficients of
+// the seed 2 dL/dI = c0 + cI I + cT T with dL/dI = (2 s/N)(s I - T) - beta/N.
+__global__ void __launch_bounds__(1024) simse_reduce_kernel(const double* __restrict__ scratch, long long tiles, int n_lambda,
+                                                            double npts, double beta, float* __restrict__ coef,
+                                                            double* __restrict__ out)
+{
+    __shared__ double sh[4][1024];
+    double total = 0.0;
+    for (int lam = 0; lam < n_lambda; ++lam) {
+        double a[4] = {0.0, 0.0, 0.0, 0.0};
+        const double* sc = scratch + 4 * tiles * lam;
+        for (long long i = threadIdx.x; i < tiles; i += 1024)
+            for (int k = 0; k < 4; ++k) a[k] += sc[4 * i + k];
+        for (int k = 0; k < 4; ++k) sh[k][threadIdx.x] = a[k];
+        __syncthreads();
+        for (int d = 512; d > 0; d >>= 1) {
+            if ((int)threadIdx.x < d)
+                for (int k = 0; k < 4; ++k) sh[k][threadIdx.x] += sh[k][threadIdx.x + d];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) {
+            const double it = sh[0][0], ii = sh[1][0], si = sh[2][0], tt = sh[3][0];
+            const double s = ii > 0.0 ? it / ii : 0.0;
+            total += (tt - s * it) / npts + beta * (1.0 - si / npts);
+            coef[4 * lam + 0] = (float)(-2.0 * beta / npts);
+            coef[4 * lam + 1] = (float)(4.0 * s * s / npts);
+            coef[4 * lam + 2] = (float)(-4.0 * s / npts);
+            coef[4 * lam + 3] = (float)s;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0 && out != nullptr) *out = total;
+}
+
+cudaError_t launch_simse_reduce(const double* scratch, long long tiles, int n_lambda, double npts, double beta,
+                                float* coef, double* d_loss, cudaStream_t stream)
+{
+    simse_reduce_kernel<<<1, 1024, 0, stream>>>(scratch, tiles, n_lambda, npts, beta, coef, d_loss);
+    return cudaGetLastError();
+}
+
+// Rows of the x-pooled plane [cny r][cnx] -> coarse gradient [cny][cnx] (fixed order over the r rows: with the
+// lane tree of the store this is the deterministic r x r sum-pool, the adjoint of the nearest up-sampling), and
+// optionally the Adam step on the coarse fp32 layout.
+__global__ void __launch_bounds__(256) pool_rows_kernel(const float* __restrict__ xpool, float* __restrict__ grad,
+                                                        long long cny, long long cnx, int r, int with_adam, AdamParams ap,
+                                                        float* __restrict__ layout, float* __restrict__ m,
+                                                        float* __restrict__ v)
+{
+    const long long n = cny * cnx;
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) {
+        const long long Y = i / cnx, X = i - Y * cnx;
+        float g = 0.0f;
+        for (int dy = 0; dy < r; ++dy) g += xpool[(Y * r + dy) * cnx + X];
+        grad[i] = g;
+        if (with_adam) {
+            const float mn = ap.b1 * m[i] + ap.c1 * g;
+            const float vn = ap.b2 * v[i] + ap.c2 * g * g;
+            m[i] = mn;
+            v[i] = vn;
+            layout[i] = layout[i] - ap.a1 * mn / (sqrtf(vn * ap.rb2) + ap.eps);
+        }
+    }
+}
+
+cudaError_t launch_pool_rows(const float* xpool, float* grad, long long cny, long long cnx, int r, const AdamParams* adam,
+                             float* layout, float* m, float* v, cudaStream_t stream)
+{
+    const long long n = cny * cnx;
+    const unsigned blocks = (unsigned)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    pool_rows_kernel<<<blocks, 256, 0, stream>>>(xpool, grad, cny, cnx, r, adam != nullptr, adam ? *adam : AdamParams{},
+                                                 layout, m, v);
+    return cudaGetLastError();
+}
+
+__global__ void __launch_bounds__(256) adam_kernel(const float* __restrict__ grad, long long n, AdamParams ap,
+                                                   float* __restrict__ layout, float* __restrict__ m, float* __restrict__ v)
+{
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) {
+        const float g = grad[i];
+        const float mn = ap.b1 * m[i] + ap.c1 * g;
+        const float vn = ap.b2 * v[i] + ap.c2 * g * g;
+        m[i] = mn;
+        v[i] = vn;
+        layout[i] = layout[i] - ap.a1 * mn / (sqrtf(vn * ap.rb2) + ap.eps);
+    }
+}
+
+cudaError_t launch_adam(const float* grad, long long n, const AdamParams& adam, float* layout, float* m, float* v,
+                        cudaStream_t stream)
+{
+    const unsigned blocks = (unsigned)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    adam_kernel<<<blocks, 256, 0, stream>>>(grad, n, adam, layout, m, v);
     return cudaGetLastError();
 }
 

@@ -212,6 +212,12 @@ static void build_schedule(dop_plan* p)
         // seeded, partly transformed gradient field")
         p->fwd.push_back(mk(0, 0, -1, +1, LD_C64, MID_LOSS, ST_C64, "x-inv,|u|^2,loss,seed,x-fwd", 8, 8, wi ? 8 : 4));
         for (int j = 1; j < a; ++j) p->fwd.push_back(mk(0, j, +1, 0, LD_C64, MID_NONE, ST_C64, "x-fwd", 8, 8));
+    } else if (p->desc.loss == DOP_LOSS_SIMSE) {
+        // Eq. (6): the least-squares scale s needs the sums of the whole plane before the seed, so the row
+        // sandwich around the loss splits at the call boundary (as for DOP_LOSS_NONE)
+        const bool wis = (p->desc.flags & DOP_WRITE_INTENSITY) != 0;
+        p->fwd.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_C64_STATS, "x-inv,|u|^2,plane sums", 8, 8, wis ? 8 : 4));
+        p->adj.push_back(mk(0, 0, +1, 0, LD_SEED_SIMSE, MID_NONE, ST_C64, "si-mse seed,x-fwd", 8, 8, 4));
     } else {
         p->fwd.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_C64_INTENSITY, "x-inv,|u|^2", 8, 8, 4));
         p->adj.push_back(mk(0, 0, +1, 0, LD_SEED, MID_NONE, ST_C64, "seed,x-fwd", 8, 8, 4));
@@ -224,6 +230,19 @@ static void build_schedule(dop_plan* p)
         p->pre.push_back(mk(0, 0, +1, 0, LD_REAL, MID_NONE, ST_C64, "real,x-fwd", 4, 8));
         sandwich_core(p, MID_GAUSS, true, &p->pre);
         p->pre.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_REAL, "x-inv,real", 8, 4));
+    }
+    if ((p->up_lg > 0 || p->desc.layout_dtype != DOP_LAYOUT_F32) && p->pre.empty()) {
+        // super-resolved layout: the height is read from the coarse plane (hb bytes per fine point) and dL/dh
+        // leaves as the x-pooled plane (4 / r bytes per fine point).  (With the pre-filter the phase passes work
+        // on the filtered fine plane; the coarse read / pooled write then sit at the two ends of the filter.)
+        const double r = (double)(1 << p->up_lg);
+        const double hb = (p->desc.layout_dtype == DOP_LAYOUT_U8 ? 1.0 : p->desc.layout_dtype == DOP_LAYOUT_U16 ? 2.0 : 4.0) / (r * r);
+        for (std::vector<PassTmpl>* v : {&p->fwd, &p->adj})
+            for (PassTmpl& t : *v) {
+                if (t.load_op == LD_HEIGHT) t.rd = hb;
+                if (t.store_op == ST_GRAD) { t.side = hb; t.wr = 4.0 / r; }
+                t.bytes_per_point = t.rd + t.wr + t.side;
+            }
     }
     if (p->x_cluster)
         for (std::vector<PassTmpl>* v : {&p->fwd, &p->adj, &p->pre})
@@ -320,6 +339,17 @@ dop_status build_plan(dop_plan* p)
     if (!is_23_smooth(d.nx) || !is_23_smooth(d.ny)) return DOP_ERR_UNSUPPORTED_SIZE;
     const dop_tuning& tu = p->tune;
     p->force_generic = tu.force_generic != 0;
+    // ---- design-loop options
+    if (d.loss == DOP_LOSS_SIMSE && !(std::isfinite(d.energy_beta) && d.energy_beta >= 0.0)) return DOP_ERR_INVALID_ARG;
+    if (d.layout_dtype != DOP_LAYOUT_F32 && d.layout_dtype != DOP_LAYOUT_U8 && d.layout_dtype != DOP_LAYOUT_U16)
+        return DOP_ERR_INVALID_ARG;
+    if (d.layout_dtype != DOP_LAYOUT_F32 && !(std::isfinite(d.layout_step) && d.layout_step > 0.0)) return DOP_ERR_INVALID_ARG;
+    p->up_lg = 0;
+    if (d.upsample != 0 && d.upsample != 1) {
+        if (d.upsample != 2 && d.upsample != 4 && d.upsample != 8) return DOP_ERR_INVALID_ARG;
+        p->up_lg = d.upsample == 2 ? 1 : (d.upsample == 4 ? 2 : 3);
+        if (d.nx % d.upsample != 0 || d.ny % d.upsample != 0) return DOP_ERR_UNSUPPORTED_SIZE;
+    }
     if (tu.tile_pts != 0) {
         if (tu.tile_pts < 256 || tu.tile_pts > 16384) return DOP_ERR_INVALID_ARG;
         p->tile_pts = tu.tile_pts;
@@ -357,14 +387,29 @@ dop_status build_plan(dop_plan* p)
                    p->ax[0].dig[1].fast;
     if (p->x_cluster && tu.cluster_lines > 0 && !cluster_instantiated(lx[1], tu.cluster_lines)) return DOP_ERR_INVALID_ARG;
     build_schedule(p);
-    // CTAs of the MID_LOSS pass, in the geometry it is launched with (one loss partial per CTA)
+    // CTAs of the MID_LOSS / plane-sum pass, in the geometry it is launched with (partials per CTA)
     p->loss_tiles = 0;
     for (const PassTmpl& t : p->fwd)
-        if (t.mid_op == MID_LOSS) {
+        if (t.mid_op == MID_LOSS || t.store_op == ST_C64_STATS) {
             PassDesc g{};
             pass_geometry(p, t, &g);
             p->loss_tiles = g.n_cgroups * g.n_m * g.n_o;
         }
+    // The sum-pool along x is a shuffle reduction over r adjacent lanes of the register-blocked kernels: the
+    // pass that stores dL/dh (and the pre-filter's real-plane store) must be one of them, with r | its lane run
+    if (p->up_lg > 0) {
+        const int r = 1 << p->up_lg;
+        for (const std::vector<PassTmpl>* v : {&p->adj, &p->pre})
+            for (const PassTmpl& t : *v) {
+                if (t.store_op != ST_GRAD && t.store_op != ST_REAL) continue;
+                PassDesc g{};
+                pass_geometry(p, t, &g);
+                const Digit& dg = p->ax[0].dig[0];
+                bool ok = t.cluster || dg.fast;
+                if (ok && !t.cluster) ok = g.col_type ? (g.nl % r == 0 && dg.st % r == 0) : (g.L / 16 >= r && g.L % r == 0);
+                if (!ok) return DOP_ERR_UNSUPPORTED_SIZE;
+            }
+    }
     // workspace: [n_lambda fields][h_eff plane][loss partials]
     const size_t npts = (size_t)d.nx * (size_t)d.ny;
     auto align256 = [](size_t x) { return (x + 255) & ~(size_t)255; };
@@ -374,6 +419,14 @@ dop_status build_plan(dop_plan* p)
     if (d.prefilter_sigma_px > 0.0) off += align256(npts * sizeof(float));
     p->ws_loss_off = off;
     if (d.loss == DOP_LOSS_L2) off += align256((size_t)p->loss_tiles * (size_t)d.n_lambda * sizeof(double));
+    if (d.loss == DOP_LOSS_SIMSE) off += align256((size_t)p->loss_tiles * (size_t)d.n_lambda * 4 * sizeof(double));
+    p->ws_coef_off = off;
+    if (d.loss == DOP_LOSS_SIMSE) off += align256((size_t)d.n_lambda * 4 * sizeof(float));
+    p->ws_xpool_off = off;
+    if (p->up_lg > 0) off += align256(npts / (size_t)(1 << p->up_lg) * sizeof(float));
+    // pre-filter on a coarse / integer layout: A5 writes the fine dL/dh_eff plane here, the filter's adjoint pools it
+    p->ws_gfine_off = off;
+    if (d.prefilter_sigma_px > 0.0 && (p->up_lg > 0 || d.layout_dtype != DOP_LAYOUT_F32)) off += align256(npts * sizeof(float));
     p->ws_bytes = off;
     return DOP_OK;
 }
@@ -383,7 +436,9 @@ std::string describe_plan(const dop_plan* p)
     std::ostringstream os;
     const dop_plan_desc& d = p->desc;
     os << "grid ny=" << d.ny << " nx=" << d.nx << " n_lambda=" << d.n_lambda
-       << " loss=" << (d.loss == DOP_LOSS_L2 ? "L2" : "none") << " prefilter_sigma_px=" << d.prefilter_sigma_px
+       << " loss=" << (d.loss == DOP_LOSS_L2 ? "L2" : d.loss == DOP_LOSS_SIMSE ? "si-mse+energy" : "none")
+       << " upsample=" << (1 << p->up_lg) << " layout=" << (d.layout_dtype == DOP_LAYOUT_U8 ? "u8" : d.layout_dtype == DOP_LAYOUT_U16 ? "u16" : "f32")
+       << " prefilter_sigma_px=" << d.prefilter_sigma_px
        << " workspace_bytes=" << p->ws_bytes << " loss_tiles=" << p->loss_tiles << "\n";
     for (int a = 0; a < 2; ++a) {
         os << (a == 0 ? "x" : "y") << "-digits:";

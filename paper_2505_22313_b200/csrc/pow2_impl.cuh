@@ -261,6 +261,36 @@ __device__ __forceinline__ float2 apply_h_fixed(float2 v, double c_minus_fx2, do
     return make_float2(0.0f, 0.0f);
 }
 
+// Height of fine-grid point (row, x) from the caller's design layout: nearest-neighbour up-sampling of the
+// coarse feature grid (the adjoint is the sum-pool in the gradient store) and gray
+// levels times a height step.
+__device__ __forceinline__ float ld_layout(const void* base, int dtype, float step, int up_lg, long long cnx, long long row,
+                                           long long x)
+{
+    const long long ci = (row >> up_lg) * cnx + (x >> up_lg);
+    if (dtype == DOP_LAYOUT_F32) return __ldg((const float*)base + ci);
+    if (dtype == DOP_LAYOUT_U8) return step * (float)__ldg((const unsigned char*)base + ci);
+    return step * (float)__ldg((const unsigned short*)base + ci);
+}
+
+// Sum over the r = 2^up_lg adjacent lanes that hold r adjacent x (deterministic xor tree; every lane gets the sum)
+__device__ __forceinline__ float pool_lanes(float g, int up_lg, unsigned mask)
+{
+    for (int d = 1; d < (1 << up_lg); d <<= 1) g += __shfl_xor_sync(mask, g, d);
+    return g;
+}
+
+// Adam (Kingma & Ba 2014, Alg. 1) on one element: returns the updated layout value
+__device__ __forceinline__ float adam_update(float g, float h, float* m, float* v, float b1, float b2, float c1, float c2,
+                                             float a1, float rb2, float eps)
+{
+    const float mn = fmaf(b1, *m, c1 * g);
+    const float vn = fmaf(b2, *v, c2 * g * g);
+    *m = mn;
+    *v = vn;
+    return h - a1 * mn / (sqrtf(vn * rb2) + eps);
+}
+
 // ---- the tile-pass kernel -------------------------------------------------------------------
 template <int L, bool COL, int V, int TWB, int NB>
 __global__ void __launch_bounds__(tile_threads(L, COL, NB), min_blocks(L, COL, V, NB))
@@ -335,6 +365,17 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
     }
 
+    // Design-layout addressing (dop_plan_desc.upsample / layout_dtype; only the variants that touch the
+    // height plane, a real plane or dL/dh): fine-grid (row, x) of register i in the first group's layout
+    constexpr bool LAYV = V == V_HEIGHT || V == V_GRAD || V == V_LDOTHER || V == V_STOTHER;
+    const bool lay = LAYV && (p.up_lg | p.h_dtype | p.coarse_in | p.pool_out) != 0; // uniform over the grid
+    long long hrow = 0, hx0 = 0;
+    if (lay) {
+        if (COL) { hrow = o; hx0 = m * p.SM + line + (long long)tt * es; }
+        else { hrow = line / p.lpr; hx0 = (line - hrow * p.lpr) * L + tt; }
+    }
+    const long long hxs = COL ? (long long)T * es : T;
+
     // (row tiles only: on column tiles it measured as a loss or as a wash that over-fetches DRAM, and
     // its registers cost the fused variants up to 25 %)
     if (!COL)
@@ -356,6 +397,19 @@ pow2_kernel(const __grid_constant__ PassDesc p)
     // ---- load (+ prologue op, + conj boundary twiddle before an inverse DFT)
     if (DIR1 > 0) {
         long long off = b0;
+        if ((V == V_HEIGHT && lay) || (V == V_LDOTHER && p.coarse_in)) {
+            // design layout: nearest up-sampling / gray levels inside the read (kept apart from the plain loops
+            // below, whose shape the row kernels are sensitive to)
+#pragma unroll
+            for (int i = 0; i < P; ++i, off += step0) {
+                if (V == V_HEIGHT) {
+                    const float hv = ld_layout(p.height, p.h_dtype, p.h_step, p.up_lg, p.cnx, hrow, hx0 + i * hxs);
+                    sincos_turns(hv * p.phase_coef, &v[i].y, &v[i].x);
+                } else {
+                    v[i] = make_float2(ld_layout(p.plane_in, p.h_dtype, p.h_step, p.up_lg, p.cnx, hrow, hx0 + i * hxs), 0.0f);
+                }
+            }
+        } else {
 #pragma unroll
         for (int i = 0; i < P; ++i, off += step0) {
             if (V == V_HEIGHT) {
@@ -366,12 +420,18 @@ pow2_kernel(const __grid_constant__ PassDesc p)
                     const float2 u = field_ld<CG>(p.field + off);
                     const float g = 2.0f * __ldg(p.plane_in + off);
                     v[i] = make_float2(g * u.x, g * u.y);
+                } else if (p.load_op == LD_SEED_SIMSE) { // Eq. (6): 2 dL/dI = c0 + cI I + cT T
+                    const float2 u = field_ld<CG>(p.field + off);
+                    const float I = u.x * u.x + u.y * u.y;
+                    const float g = fmaf(__ldg(p.coef + 1), I, fmaf(__ldg(p.coef + 2), __ldg(p.plane_in + off), __ldg(p.coef)));
+                    v[i] = make_float2(g * u.x, g * u.y);
                 } else {
                     v[i] = make_float2(__ldg(p.plane_in + off), 0.0f);
                 }
             } else {
                 v[i] = field_ld<CG>(p.field + off);
             }
+        }
         }
     } else {
         if (STAGE) {
@@ -499,6 +559,39 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         }
     } else {
         long long off = b0;
+        double st0 = 0.0, st1 = 0.0, st2 = 0.0, st3 = 0.0; // ST_C64_STATS: <I,T>, <I,I>, sum I, <T,T>
+        if ((V == V_GRAD && (lay || p.adam_m != nullptr)) || (V == V_STOTHER && p.pool_out)) {
+            // design-loop flavours of the two real-plane stores (kept apart from the plain loops below)
+            const unsigned am = __activemask();
+            const bool leader = ((COL ? sub : tt) & ((1 << p.up_lg) - 1)) == 0;
+#pragma unroll
+            for (int i = 0; i < P; ++i, off += step0) {
+                if (V == V_GRAD) {
+                    const float hv = lay ? ld_layout(p.height, p.h_dtype, p.h_step, p.up_lg, p.cnx, hrow, hx0 + i * hxs)
+                                         : __ldg(p.height + off);
+                    float sn, cs;
+                    sincos_turns(hv * p.phase_coef, &sn, &cs);
+                    float g = p.grad_coef * (cs * v[i].y - sn * v[i].x); // A5: c Im(conj(u0) g)
+                    if (p.pool_out) { // adjoint of the nearest up-sampling along x; rows are pooled afterwards
+                        g = pool_lanes(g, p.up_lg, am);
+                        const long long ci = hrow * p.cnx + ((hx0 + i * hxs) >> p.up_lg);
+                        if (leader) {
+                            if (p.store_op == ST_GRAD_ACC) g += p.plane_out[ci];
+                            p.plane_out[ci] = g;
+                        }
+                    } else {
+                        if (p.store_op == ST_GRAD_ACC) g += __ldg(p.plane_out + off);
+                        p.plane_out[off] = g;
+                        if (p.adam_m != nullptr) // the optimiser step rides on the last wavelength's store
+                            p.adam_h[off] = adam_update(g, hv, p.adam_m + off, p.adam_v + off, p.adam_b1, p.adam_b2, p.adam_c1,
+                                                        p.adam_c2, p.adam_a1, p.adam_rb2, p.adam_eps);
+                    }
+                } else {
+                    const float g = pool_lanes(v[i].x, p.up_lg, am);
+                    if (leader) p.plane_out[hrow * p.cnx + ((hx0 + i * hxs) >> p.up_lg)] = g;
+                }
+            }
+        } else {
 #pragma unroll
         for (int i = 0; i < P; ++i, off += step0) {
             if (V == V_GRAD) {
@@ -512,11 +605,46 @@ pow2_kernel(const __grid_constant__ PassDesc p)
                 if (p.store_op == ST_C64_INTENSITY) {
                     field_st<CG>(p.field + off, v[i]);
                     p.plane_out[off] = v[i].x * v[i].x + v[i].y * v[i].y;
+                } else if (p.store_op == ST_C64_STATS) {
+                    field_st<CG>(p.field + off, v[i]);
+                    const float I = v[i].x * v[i].x + v[i].y * v[i].y;
+                    const float Tv = __ldg(p.plane_in + off);
+                    st0 += (double)I * (double)Tv;
+                    st1 += (double)I * (double)I;
+                    st2 += (double)I;
+                    st3 += (double)Tv * (double)Tv;
+                    if (p.write_intensity) p.plane_out[off] = I;
                 } else {
                     p.plane_out[off] = v[i].x;
                 }
             } else {
                 field_st<CG>(p.field + off, v[i]);
+            }
+        }
+        }
+        if (V == V_STOTHER) {
+            if (p.store_op == ST_C64_STATS) { // deterministic CTA reduction of the four plane sums
+                __shared__ double sred[4][32];
+                constexpr int NT = tile_threads(L, COL, NB);
+                constexpr int SW = NT < 32 ? NT : 32;
+                constexpr unsigned SMASK = NT < 32 ? (1u << SW) - 1u : 0xffffffffu;
+#pragma unroll
+                for (int d = SW / 2; d > 0; d >>= 1) {
+                    st0 += __shfl_down_sync(SMASK, st0, d, SW);
+                    st1 += __shfl_down_sync(SMASK, st1, d, SW);
+                    st2 += __shfl_down_sync(SMASK, st2, d, SW);
+                    st3 += __shfl_down_sync(SMASK, st3, d, SW);
+                }
+                if ((tid & 31) == 0) {
+                    sred[0][tid >> 5] = st0; sred[1][tid >> 5] = st1; sred[2][tid >> 5] = st2; sred[3][tid >> 5] = st3;
+                }
+                __syncthreads();
+                if (tid < 4) {
+                    double r = 0.0;
+                    constexpr int NW = (NT + 31) / 32;
+                    for (int w = 0; w < NW; ++w) r += sred[tid][w];
+                    p.loss_scratch[4 * (p.tile0 + blockIdx.x) + tid] = r;
+                }
             }
         }
     }

@@ -22,7 +22,12 @@ DOP_ERR_ARCH = 5
 DOP_ERR_CUDA = 6
 DOP_LOSS_NONE = 0
 DOP_LOSS_L2 = 1
+DOP_LOSS_SIMSE = 2
+DOP_LAYOUT_F32 = 0
+DOP_LAYOUT_U8 = 1
+DOP_LAYOUT_U16 = 2
 DOP_WRITE_INTENSITY = 0x1
+_LAYOUT_TORCH = {DOP_LAYOUT_F32: torch.float32, DOP_LAYOUT_U8: torch.uint8, DOP_LAYOUT_U16: torch.uint16}
 
 
 class dop_tuning(C.Structure):
@@ -41,7 +46,13 @@ class dop_plan_desc(C.Structure):
         ("lambda_", C.POINTER(C.c_double)), ("n_refr", C.POINTER(C.c_double)), ("z", C.c_double),
         ("loss", C.c_int), ("prefilter_sigma_px", C.c_double), ("flags", C.c_uint32),
         ("tuning", C.POINTER(dop_tuning)),
+        ("energy_beta", C.c_double), ("upsample", C.c_int32), ("layout_dtype", C.c_int32), ("layout_step", C.c_double),
     ]
+
+
+class dop_adam(C.Structure):
+    _fields_ = [("lr0", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("eps", C.c_double),
+                ("iter", C.c_int64), ("total_iters", C.c_int64)]
 
 
 def make_tuning(xdigits: Sequence[int] = (), ydigits: Sequence[int] = (), **fields) -> dop_tuning:
@@ -78,6 +89,8 @@ def _load() -> C.CDLL:
     lib.dop_propagate_fwd.restype = C.c_int
     lib.dop_propagate_adj.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.dop_propagate_adj.restype = C.c_int
+    lib.dop_propagate_adj_adam.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(dop_adam), vp, vp]
+    lib.dop_propagate_adj_adam.restype = C.c_int
     lib.dop_plan_destroy.argtypes = [vp]
     lib.dop_plan_destroy.restype = C.c_int
     lib.dop_status_string.argtypes = [C.c_int]
@@ -96,7 +109,7 @@ def _load() -> C.CDLL:
 
 
 _lib = _load()
-EXPORTS = ("dop_plan_create", "dop_propagate_fwd", "dop_propagate_adj", "dop_plan_destroy",
+EXPORTS = ("dop_plan_create", "dop_propagate_fwd", "dop_propagate_adj", "dop_propagate_adj_adam", "dop_plan_destroy",
            "dop_status_string", "dop_plan_describe", "dop_plan_launch_count",
            "dop_plan_set_profiling", "dop_plan_get_pass_times", "dop_plan_pass_name")
 
@@ -116,14 +129,16 @@ def _ptr(t: Optional[torch.Tensor], dtype, what: str) -> Optional[int]:
 
 def dop_plan_create(ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
                     z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0,
-                    tuning: Optional[dop_tuning] = None):
+                    tuning: Optional[dop_tuning] = None, energy_beta: float = 0.0, upsample: int = 0,
+                    layout_dtype: int = DOP_LAYOUT_F32, layout_step: float = 0.0):
     """-> (plan handle, workspace_bytes).  Host-only; raises DopError on a bad description."""
     nl = len(lambdas)
     lam = (C.c_double * max(nl, 1))(*[float(v) for v in lambdas])
     nr = (C.c_double * max(nl, 1))(*[float(v) for v in n_refr])
     d = dop_plan_desc(int(ny), int(nx), float(pitch), nl, lam, nr, float(z), int(loss),
                       float(prefilter_sigma_px), int(flags),
-                      C.pointer(tuning) if tuning is not None else None)
+                      C.pointer(tuning) if tuning is not None else None,
+                      float(energy_beta), int(upsample), int(layout_dtype), float(layout_step))
     out, ws = C.c_void_p(), C.c_size_t(0)
     st = _lib.dop_plan_create(C.byref(out), C.byref(d), C.byref(ws))
     if st != DOP_OK:
@@ -138,8 +153,8 @@ def _stream(stream) -> int:
 
 
 def dop_propagate_fwd(plan, d_height, d_target=None, d_intensity=None, d_loss=None, d_workspace=None,
-                      stream=None) -> None:
-    st = _lib.dop_propagate_fwd(plan, _ptr(d_height, torch.float32, "d_height"),
+                      stream=None, layout_dtype: int = DOP_LAYOUT_F32) -> None:
+    st = _lib.dop_propagate_fwd(plan, _ptr(d_height, _LAYOUT_TORCH[layout_dtype], "d_height"),
                                 _ptr(d_target, torch.float32, "d_target"),
                                 _ptr(d_intensity, torch.float32, "d_intensity"),
                                 _ptr(d_loss, torch.float64, "d_loss"),
@@ -148,13 +163,25 @@ def dop_propagate_fwd(plan, d_height, d_target=None, d_intensity=None, d_loss=No
         raise DopError(st, "dop_propagate_fwd")
 
 
-def dop_propagate_adj(plan, d_height, d_dLdI=None, d_grad_height=None, d_workspace=None, stream=None) -> None:
-    st = _lib.dop_propagate_adj(plan, _ptr(d_height, torch.float32, "d_height"),
+def dop_propagate_adj(plan, d_height, d_dLdI=None, d_grad_height=None, d_workspace=None, stream=None,
+                      layout_dtype: int = DOP_LAYOUT_F32) -> None:
+    st = _lib.dop_propagate_adj(plan, _ptr(d_height, _LAYOUT_TORCH[layout_dtype], "d_height"),
                                 _ptr(d_dLdI, torch.float32, "d_dLdI"),
                                 _ptr(d_grad_height, torch.float32, "d_grad_height"),
                                 None if d_workspace is None else d_workspace.data_ptr(), _stream(stream))
     if st != DOP_OK:
         raise DopError(st, "dop_propagate_adj")
+
+
+def dop_propagate_adj_adam(plan, d_layout, d_dLdI, d_grad_height, d_m, d_v, lr0: float, beta1: float, beta2: float,
+                           eps: float, it: int, total_iters: int, d_workspace=None, stream=None) -> None:
+    hp = dop_adam(float(lr0), float(beta1), float(beta2), float(eps), int(it), int(total_iters))
+    st = _lib.dop_propagate_adj_adam(plan, _ptr(d_layout, torch.float32, "d_layout"), _ptr(d_dLdI, torch.float32, "d_dLdI"),
+                                     _ptr(d_grad_height, torch.float32, "d_grad_height"), _ptr(d_m, torch.float32, "d_m"),
+                                     _ptr(d_v, torch.float32, "d_v"), C.byref(hp),
+                                     None if d_workspace is None else d_workspace.data_ptr(), _stream(stream))
+    if st != DOP_OK:
+        raise DopError(st, "dop_propagate_adj_adam")
 
 
 def dop_plan_destroy(plan) -> None:
@@ -194,10 +221,13 @@ class Plan:
 
     def __init__(self, ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
                  z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0,
-                 device: str = "cuda:0", tuning: Optional[dop_tuning] = None):
+                 device: str = "cuda:0", tuning: Optional[dop_tuning] = None, energy_beta: float = 0.0,
+                 upsample: int = 0, layout_dtype: int = DOP_LAYOUT_F32, layout_step: float = 0.0):
         self.ny, self.nx, self.n_lambda, self.loss, self.flags = int(ny), int(nx), len(lambdas), loss, flags
+        self.layout_dtype = layout_dtype
         self.handle, self.workspace_bytes = dop_plan_create(ny, nx, pitch, lambdas, n_refr, z, loss,
-                                                            prefilter_sigma_px, flags, tuning)
+                                                            prefilter_sigma_px, flags, tuning, energy_beta, upsample,
+                                                            layout_dtype, layout_step)
         self.device = torch.device(device)
         self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
         self.launches = dop_plan_launch_count(self.handle)
@@ -206,10 +236,14 @@ class Plan:
         return dop_plan_describe(self.handle)
 
     def fwd(self, height, target=None, intensity=None, loss=None, stream=None) -> None:
-        dop_propagate_fwd(self.handle, height, target, intensity, loss, self.workspace, stream)
+        dop_propagate_fwd(self.handle, height, target, intensity, loss, self.workspace, stream, self.layout_dtype)
 
     def adj(self, height, dLdI=None, grad=None, stream=None) -> None:
-        dop_propagate_adj(self.handle, height, dLdI, grad, self.workspace, stream)
+        dop_propagate_adj(self.handle, height, dLdI, grad, self.workspace, stream, self.layout_dtype)
+
+    def adj_adam(self, layout, dLdI, grad, m, v, lr0, beta1, beta2, eps, it, total_iters, stream=None) -> None:
+        dop_propagate_adj_adam(self.handle, layout, dLdI, grad, m, v, lr0, beta1, beta2, eps, it, total_iters,
+                               self.workspace, stream)
 
     def field(self) -> torch.Tensor:
         """complex64 view [n_lambda, ny, nx] of the workspace fields (valid after a DOP_LOSS_NONE fwd)."""
