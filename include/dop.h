@@ -109,7 +109,11 @@ typedef struct {
     int32_t cluster_force;  /* != 0: cluster row kernels wherever they exist (nx = 16384, 32768, 65536);  */
                             /*       by default only where measured faster than two digit passes          */
                             /*       (nx = 16384, clusters of 2; profiles/r02_cluster.md)                 */
-    int32_t reserved[4];    /* must be 0                                                                */
+    int32_t no_tma;         /* != 0: column passes through the LDG/STG kernels (pow2_impl.cuh) instead of the   */
+                            /*       persistent TMA pipeline (tma_col.cuh)                                      */
+    int32_t tma_nb;         /* 16 | 32: columns per TMA tile (0 = per-pass default)                              */
+    int32_t tma_stages;     /* 1..8: tiles in flight per CTA of the TMA kernels (0 = per-pass default)          */
+    int32_t reserved[1];    /* must be 0                                                                */
 } dop_tuning;
 
 typedef struct {

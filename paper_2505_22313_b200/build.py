@@ -22,8 +22,11 @@ SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu"]
 POW2_INST = [(1, L) for L in (16, 32, 64, 128, 256, 512)] + \
             [(0, L) for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192)]
 POW2_X3 = (16, 32, 64, 128)  # digits 3 * LP
+# (digit length, bundle width, pipeline depth) of the TMA column kernels -- must match DOP_TMA_LIST in kernels_pow2.cu
+TMA_INST = [(64, 32, 3), (64, 16, 3), (128, 32, 3), (128, 16, 3), (256, 32, 2), (256, 16, 3), (256, 16, 2), (512, 16, 2),
+            (96, 32, 3), (192, 32, 3), (384, 32, 2)]
 CLUSTER_INST = [(4096, 2), (4096, 1), (2048, 4), (1024, 8)]  # (local transform length M, lines per CTA S): rows of 16 M
-HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", "cluster_row.cuh", os.path.join("..", "..", "include", "dop.h")]
+HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", "cluster_row.cuh", "tma_col.cuh", os.path.join("..", "..", "include", "dop.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC",
@@ -43,6 +46,9 @@ def _units():
     for m, sl in CLUSTER_INST:
         units.append((os.path.join(OBJDIR, f"cluster_{m}_{sl}.o"), os.path.join(CSRC, "cluster_inst.cu"),
                       [f"-DDOP_INST_CLUSTER_M={m}", f"-DDOP_INST_CLUSTER_S={sl}"]))
+    for L, nb, nst in TMA_INST:
+        units.append((os.path.join(OBJDIR, f"tma_{L}_{nb}_{nst}.o"), os.path.join(CSRC, "tma_inst.cu"),
+                      [f"-DDOP_INST_TMA_L={L}", f"-DDOP_INST_TMA_NB={nb}", f"-DDOP_INST_TMA_NST={nst}"]))
     for lp in POW2_X3:
         units.append((os.path.join(OBJDIR, f"pow2_x3_{lp}.o"), os.path.join(CSRC, "pow2_inst.cu"),
                       [f"-DDOP_INST_X3={lp}"]))
@@ -54,7 +60,7 @@ def _units():
 
 def _dep_stamp() -> str:
     h = hashlib.sha256()
-    for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS + ["pow2_inst.cu", "cluster_inst.cu"]] + [os.path.abspath(__file__)]:
+    for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS + ["pow2_inst.cu", "cluster_inst.cu", "tma_inst.cu"]] + [os.path.abspath(__file__)]:
         with open(d, "rb") as f:
             h.update(f.read())
     h.update((" ".join(NVCC_FLAGS) + os.environ.get("DOP_NVCC_EXTRA", "")).encode())

@@ -114,7 +114,9 @@ dop_status ensure_device(dop_plan* p)
 PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b, char* ws)
 {
     PassDesc d{};
-    pass_geometry(p, t, &d);
+    // (the TMA kernels implement neither the dL/dh accumulate of later wavelengths nor the fused Adam store)
+    const bool tma_ok = !(t.store_op == ST_GRAD && (lam > 0 || (b.adam != nullptr && lam == p->desc.n_lambda - 1) || b.grad_pool));
+    pass_geometry(p, t, &d, tma_ok);
     // (a cluster pass takes its group twiddles from x digit 1 and its boundary twiddles from x digit 0)
     const Digit& g = p->ax[t.axis].dig[(size_t)(t.cluster ? 1 : t.digit)];
     char* arena = (char*)p->d_arena;
@@ -197,6 +199,12 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.inv_lam2 = 1.0 / (lambda * lambda);
     d.z = p->desc.z;
     d.h_fixed = (std::fabs(p->desc.z) / lambda < 524288.0 && !p->h_float) ? 1 : 0;
+    {
+        const double sc = 1.0 / (double)npts, tp = 2.0 * M_PI;
+        const double sk[5] = {tp, -tp * tp * tp / 6.0, std::pow(tp, 5) / 120.0, -std::pow(tp, 7) / 5040.0, std::pow(tp, 9) / 362880.0};
+        const double ck[5] = {1.0, -tp * tp / 2.0, std::pow(tp, 4) / 24.0, -std::pow(tp, 6) / 720.0, std::pow(tp, 8) / 40320.0};
+        for (int q = 0; q < 5; ++q) { d.hk_s[q] = (float)(sc * sk[q]); d.hk_c[q] = (float)(sc * ck[q]); }
+    }
     // prefetch distance in tiles: pf_waves x (148 SMs x resident CTAs of ~1024 threads per SM)
     {
         const long long threads = d.cluster ? 512 : (d.col_type ? d.L : (long long)d.nl * d.L / 16);

@@ -104,6 +104,7 @@ struct PassDesc {
     float scale;          // 1/(ny nx)
     float seed_coef;      // 4/(ny nx)
     double inv_lam2, z;   // H
+    float hk_s[5], hk_c[5]; // scale (2 pi)^n/n! with signs: sine / cosine polynomial of H in the TMA kernels (apply_h_fixed_nb)
     int h_fixed;          // pow2 kernels: |z|/lambda < 2^19, the phase of H may be taken in 32-bit fixed point
     const double* fx2;    // [nx] slot -> fx^2   (fp64, same expression as the definition)
     const double* fy2;    // [ny] slot -> fy^2
@@ -114,6 +115,7 @@ struct PassDesc {
     int threads;
     int cluster;          // 1 (exchange through L2) | 2 (through DSMEM) = cluster row pass (cluster_row.cuh): L = M, the x digits (16, M) fused; n_o rows
     int device;           // the plan's device (function attributes are set once per device)
+    int tma;              // > 0: TMA column kernel (tma_col.cuh) with this many tiles in flight per CTA; nl = its bundle width
 };
 
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream);
@@ -122,6 +124,7 @@ bool pow2_supported(long long L, bool col_type);
 bool cluster_supported(long long L0, long long L1);
 int cluster_size(long long L1);
 bool cluster_instantiated(long long L1, int lines);
+bool tma_instantiated(long long L, int nb, int nst);
 int pow2_lines(long long L, bool col_type, bool plain = false, int nb_override = 0);
 std::vector<float2> pow2_group_twiddles(long long L);
 cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
@@ -195,6 +198,8 @@ struct dop_plan {
     long long slab_bytes = 0;   // L2 slab size for multi-pass segments (0 = whole-array launches)
     bool force_generic = false; // dop_tuning.force_generic: generic kernel for every pass
     bool x_cluster = false;     // the x digits are (16, M) and run as one cluster pass
+    bool use_tma = true;        // column passes through the TMA kernels where instantiated (dop_tuning.no_tma)
+    int tma_nb = 0, tma_stages = 0; // dop_tuning overrides of their bundle width / pipeline depth (0 = default)
     // schedules for one lambda
     std::vector<dop::PassTmpl> fwd, adj, pre; // pre = Gaussian pre-filter (real -> real)
     long long loss_tiles = 0;                 // CTAs of the MID_LOSS pass
@@ -228,5 +233,5 @@ namespace dop {
 dop_status build_plan(dop_plan* p);
 std::string describe_plan(const dop_plan* p);
 void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d);
-void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d);
+void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow_tma = true);
 } // namespace dop

@@ -3,6 +3,7 @@
 #include <cstdlib>
 
 #include "cluster_row.cuh"
+#include "tma_col.cuh"
 
 namespace dop {
 
@@ -21,6 +22,76 @@ extern template cudaError_t launch_x3<16>(const PassDesc&, int, int, cudaStream_
 extern template cudaError_t launch_x3<32>(const PassDesc&, int, int, cudaStream_t);
 extern template cudaError_t launch_x3<64>(const PassDesc&, int, int, cudaStream_t);
 extern template cudaError_t launch_x3<128>(const PassDesc&, int, int, cudaStream_t);
+
+// TMA column kernels (tma_col.cuh): (digit length, bundle width, pipeline depth) instantiated in the tma_inst.cu
+// objects -- the same list as TMA_INST in build.py
+#define DOP_TMA_LIST(X) \
+    X(64, 32, 3) X(64, 16, 3) X(128, 32, 3) X(128, 16, 3) X(256, 32, 2) X(256, 16, 3) X(256, 16, 2) X(512, 16, 2) \
+    X(96, 32, 3) X(192, 32, 3) X(384, 32, 2)
+#define DOP_TMA_DECL(L, NB, NST) extern template cudaError_t launch_tma<L, NB, NST>(const PassDesc&, int, int, cudaStream_t);
+DOP_TMA_LIST(DOP_TMA_DECL)
+#undef DOP_TMA_DECL
+
+bool tma_instantiated(long long L, int nb, int nst)
+{
+#define DOP_TMA_HAS(LL, NB, NST) if (L == LL && nb == NB && nst == NST) return true;
+    DOP_TMA_LIST(DOP_TMA_HAS)
+#undef DOP_TMA_HAS
+    return false;
+}
+
+TmaEncodeFn tma_encode_fn()
+{
+    static TmaEncodeFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            f = nullptr;
+        return (TmaEncodeFn)f;
+    }();
+    return fn;
+}
+
+int tma_sm_count(int device)
+{
+    static std::atomic<int> sms[64];
+    if (device < 0 || device >= 64) return 148;
+    int n = sms[device].load();
+    if (n == 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || n < 1) n = 148;
+        sms[device].store(n);
+    }
+    return n;
+}
+
+bool tma_make_map(CUtensorMap* map, const void* base, int eb, const PassDesc& p, int nb, int lb)
+{
+    TmaEncodeFn enc = tma_encode_fn();
+    if (enc == nullptr || base == nullptr || ((uintptr_t)base & 15) != 0) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)p.NC, (cuuint64_t)p.n_m, (cuuint64_t)p.L, (cuuint64_t)(p.n_o + p.o0)};
+    cuuint64_t strides[3] = {(cuuint64_t)p.SM * eb, (cuuint64_t)p.es * eb, (cuuint64_t)p.SO * eb};
+    for (int i = 0; i < 3; ++i) {
+        if (dims[i + 1] == 1 && strides[i] == 0) strides[i] = 16; // (a dimension of extent 1: the stride is never used)
+        if (strides[i] % 16 != 0 || strides[i] >= (1ull << 40)) return false;
+    }
+    for (int i = 0; i < 4; ++i)
+        if (dims[i] == 0 || dims[i] > 0xffffffffull) return false;
+    const cuuint32_t box[4] = {(cuuint32_t)nb, 1, (cuuint32_t)lb, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUtensorMapDataType dt = eb == 8 ? CU_TENSOR_MAP_DATA_TYPE_UINT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const CUtensorMapL2promotion promo = nb * eb >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+    return enc(map, dt, 4, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+static cudaError_t launch_tma_pass(const PassDesc& p, int v, int twb, cudaStream_t stream)
+{
+#define DOP_TMA_CASE(LL, NB, NST) if (p.L == LL && p.nl == NB && p.tma == NST) return launch_tma<LL, NB, NST>(p, v, twb, stream);
+    DOP_TMA_LIST(DOP_TMA_CASE)
+#undef DOP_TMA_CASE
+    return kNotInstantiated;
+}
 
 bool pow2_supported(long long L, bool col_type)
 {
@@ -111,6 +182,13 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
         twb = p.r_from == 1 ? TWB_TILE : TWB_LANE;
     }
     cudaError_t e = kNotInstantiated;
+    if (p.tma > 0 && col) { // the plan only marks passes whose variant the TMA kernels implement
+        e = launch_tma_pass(p, v, twb, stream);
+        if (e != kNotInstantiated) {
+            *handled = true;
+            return e;
+        }
+    }
     if (p.L % 3 == 0) {
         switch (p.L / 3) {
         case 16: e = launch_x3<16>(p, v, twb, stream); break;

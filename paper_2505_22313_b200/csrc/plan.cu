@@ -296,7 +296,7 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
 // is a property of the pass (it does not change where data lives): plain forward / inverse
 // passes (and the exp(i Phi) pass of short digits) take wider bundles (pow2_lines), the register-heavy fused
 // variants stay at 16 columns.
-void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d)
+void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow_tma)
 {
     if (t.cluster) { // one cluster of C CTAs per row; CTA = S lines of M points
         const long long M = p->ax[0].dig[1].L;
@@ -318,6 +318,53 @@ void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d)
     tile_geometry(p, t.axis, t.digit, d);
     const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
     if (!g.fast || !d->col_type) return;
+    // Column passes the TMA kernels implement (tma_col.cuh) run there: bundle width and pipeline depth per
+    // digit length and variant (measured, profiles/r02_tma_col.md), dop_tuning.tma_nb / tma_stages override.
+    if (allow_tma && p->use_tma) {
+        const bool x3 = g.L % 3 == 0;
+        const bool plain_layout = p->up_lg == 0 && p->desc.layout_dtype == DOP_LAYOUT_F32;
+        const bool sandwich = t.fft1_dir > 0 && t.fft2_dir < 0 && t.load_op == LD_C64 && t.store_op == ST_C64 &&
+                              (t.mid_op == MID_H || t.mid_op == MID_HCONJ || t.mid_op == MID_GAUSS);
+        const bool plainpass = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_C64 && t.store_op == ST_C64;
+        const bool lossp = t.mid_op == MID_LOSS && t.fft1_dir < 0 && t.fft2_dir > 0 && t.load_op == LD_C64 && t.store_op == ST_C64;
+        const bool heightp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_HEIGHT && t.store_op == ST_C64 && plain_layout;
+        const bool gradp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_C64 && t.store_op == ST_GRAD && plain_layout;
+        const bool has_plane = lossp || heightp || gradp;
+        // (the TMA (x) H kernel takes the phase in 32-bit fixed point: |z|/lambda < 2^19 for every wavelength)
+        bool h_ok = !p->h_float;
+        for (double lam : p->lambda) h_ok = h_ok && std::fabs(p->desc.z) / lam < 524288.0;
+        const bool sandwich_ok = sandwich && (t.mid_op == MID_GAUSS || h_ok);
+        if (plainpass || (!x3 && (sandwich_ok || has_plane))) {
+            // measured per variant at L = 256 (C4): plain passes and the dL/dh store are near the pattern's ceiling
+            // with 32-column tiles, the register-heavy fused variants want 16 columns (two CTAs per SM)
+            int nb = 32, nst = g.L <= 128 ? 3 : 2;
+            if (sandwich || lossp) { nb = 16; nst = 3; }
+            if (heightp) { nb = 16; nst = g.L == 256 ? 2 : 3; }
+            if (g.L == 512) { nb = 16; nst = 2; }
+            if (x3) { nb = 32; nst = g.L == 384 ? 2 : 3; }
+            if (p->tma_nb) nb = p->tma_nb;
+            if (p->tma_stages) nst = p->tma_stages;
+            auto fits = [&](int b, int n) {
+                return tma_instantiated(g.L, b, n) && d->NC % b == 0 &&
+                       (long long)n * g.L * b * (has_plane ? 12 : 8) <= 227 * 1024 - 2048;
+            };
+            if (!fits(nb, nst)) { // nearest instantiated choice
+                bool found = false;
+                for (int n = nst; n >= 1 && !found; --n)
+                    for (int b : {nb, 16, 32})
+                        if (fits(b, n)) { nb = b; nst = n; found = true; break; }
+                if (!found) nst = 0;
+            }
+            if (nst > 0) {
+                d->tma = nst;
+                d->nl = nb;
+                d->n_cgroups = d->NC / nb;
+                d->smem_bytes = (int)((long long)nst * g.L * nb * (has_plane ? 12 : 8));
+                d->threads = (int)(nb * (g.L / 16) + 32);
+                return;
+            }
+        }
+    }
     // (the exp(i Phi) pass: measured better at 32 columns for L = 128, worse for L = 256)
     // and the gradient / real-plane stores: +5-10 % at 32 columns for L = 128, no change for L = 256)
     const bool short_digit = g.L <= 128;
@@ -365,8 +412,12 @@ dop_status build_plan(dop_plan* p)
     // default: measured slower than whole-array launches on B200.
     if (tu.slab_mb < 0 || tu.slab_mb > 4096) return DOP_ERR_INVALID_ARG;
     p->slab_bytes = (long long)tu.slab_mb << 20;
-    for (int i = 0; i < 4; ++i)
-        if (tu.reserved[i] != 0) return DOP_ERR_INVALID_ARG;
+    if (tu.reserved[0] != 0) return DOP_ERR_INVALID_ARG;
+    if (tu.tma_nb != 0 && tu.tma_nb != 16 && tu.tma_nb != 32 && tu.tma_nb != 64) return DOP_ERR_INVALID_ARG;
+    if (tu.tma_stages < 0 || tu.tma_stages > 8) return DOP_ERR_INVALID_ARG;
+    p->use_tma = !tu.no_tma && !p->force_generic;
+    p->tma_nb = tu.tma_nb;
+    p->tma_stages = tu.tma_stages;
     if (tu.cluster_lines != 0 && tu.cluster_lines != 1 && tu.cluster_lines != 2 && tu.cluster_lines != 4 && tu.cluster_lines != 8)
         return DOP_ERR_INVALID_ARG;
     // generic kernel limits: a row-type line <= 8192 points (64 KiB), a column-type digit
@@ -458,7 +509,8 @@ std::string describe_plan(const dop_plan* p)
                 os << tag << " x0+x1 L=16x" << g.L << " tile=" << g.nl << "x" << g.L << " row cluster=" << g.n_cgroups;
             else
                 os << tag << " " << (t.axis == 0 ? "x" : "y") << t.digit << " L=" << g.L << " tile=" << g.nl << "x" << g.L
-                   << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? " pow2" : " generic");
+                   << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? (g.tma ? " tma" : " pow2") : " generic");
+            if (g.tma) os << " stages=" << g.tma;
             os << " ctas=" << g.n_cgroups * g.n_m * g.n_o
                << " smem=" << g.smem_bytes << " B/pt=" << t.bytes_per_point << " [" << t.name << "]\n";
             total += t.bytes_per_point;

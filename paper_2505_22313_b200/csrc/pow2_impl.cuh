@@ -261,6 +261,46 @@ __device__ __forceinline__ float2 apply_h_fixed(float2 v, double c_minus_fx2, do
     return make_float2(0.0f, 0.0f);
 }
 
+// Branch-free flavour of apply_h_fixed for kernels with registers to spare (tma_col.cuh): no divergent region
+// around a point's chain, so the 16 chains of a thread interleave (ncu: the branchy form sits at 52 % issue
+// utilisation with `wait` and `long_scoreboard` on top).  a < 0 runs the same arithmetic on garbage and the
+// result is replaced by 0 with two selects; a == 0 gives s = a y = 0 exactly for any finite seed, i.e. H = 1.
+// The 1/(ny nx) scale is folded into the polynomial coefficients (hk, prepared on the host: hk.s[k] =
+// scale (2 pi)^(2k+1)/(2k+1)! signed, hk.c[k] likewise for the cosine), conj H into the sign of z32.
+struct HCoef { float s[5], c[5]; };
+__device__ __forceinline__ float2 apply_h_fixed_nb(float2 v, double c_minus_fx2, double fy2, double z32, const HCoef& hk)
+{
+    const double a = c_minus_fx2 - fy2;
+    const int hi = __double2hiint(a), lo = __double2loint(a);
+    const float af = __int_as_float(((hi - 0x38000000) << 3) | (int)((unsigned)lo >> 29)); // truncated (float)a, a > 0
+    const int yb = __float_as_int(rsqrtf(af));
+    const double y = __hiloint2double((yb >> 3) + 0x38000000, yb << 29);                    // exact (double)y
+    double s = a * y;
+    s = fma(fma(-s, s, a), 0.5 * y, s);
+    const unsigned ph = (unsigned)__double2loint(fma(s, z32, 6755399441055744.0));
+    const unsigned t = ph + 0x20000000u;
+    const int q = (int)(t >> 30);
+    const int ri = (int)(t & 0x3FFFFFFFu) - 0x20000000;
+    const float rf = __int_as_float(0x4B400000 + ((ri + 64) >> 7)) - 12582912.0f;
+    const float r = rf * 2.98023223876953125e-8f;
+    const float r2 = r * r;
+    float sp = fmaf(r2, hk.s[4], hk.s[3]);
+    sp = fmaf(sp, r2, hk.s[2]);
+    sp = fmaf(sp, r2, hk.s[1]);
+    sp = fmaf(sp, r2, hk.s[0]);
+    const float sn0 = sp * r;
+    float cp = fmaf(r2, hk.c[4], hk.c[3]);
+    cp = fmaf(cp, r2, hk.c[2]);
+    cp = fmaf(cp, r2, hk.c[1]);
+    const float cs0 = fmaf(cp, r2, hk.c[0]);
+    const bool odd = (q & 1) != 0;
+    const float co = odd ? sn0 : cs0, so = odd ? cs0 : sn0;
+    const bool prop = a >= 0.0; // evanescent bins are zeroed
+    const float hx = prop ? __int_as_float(__float_as_int(co) ^ (((q + 1) & 2) << 30)) : 0.0f;
+    const float hy = prop ? __int_as_float(__float_as_int(so) ^ ((q & 2) << 30)) : 0.0f;
+    return fx::cmul(v, make_float2(hx, hy));
+}
+
 // Height of fine-grid point (row, x) from the caller's design layout: nearest-neighbour up-sampling of the
 // coarse feature grid (the adjoint is the sum-pool in the gradient store) and gray
 // levels times a height step.

@@ -147,16 +147,22 @@ def test_launch_count_follows_the_slab_schedule():
     assert n == 13 * 16 + 1
 
 
-@pytest.mark.parametrize("ny,nx,yd,xd,expect", [
-    (65536, 32, "256,256", "32", ["y0 L=256 tile=32x256 col pow2", "y1 L=256 tile=16x256 col pow2"]),
-    (16, 131072, "16", "256,512", ["x0 L=256 tile=16x256 col pow2", "x1 L=512 tile=8x512 row pow2"]),
-    (6144, 128, "384,16", "128", ["y0 L=384 tile=32x384 col pow2", "x0 L=128 tile=32x128 row pow2"]),
-    (64, 8192, "64", "8192", ["x0 L=8192 tile=1x8192 row pow2", "y0 L=64 tile=16x64 col pow2"]),
+@pytest.mark.parametrize("ny,nx,yd,xd,tun,expect", [
+    (65536, 32, "256,256", "32", {}, ["y0 L=256 tile=32x256 col tma stages=2", "y1 L=256 tile=16x256 col tma stages=3"]),
+    (65536, 32, "256,256", "32", {"no_tma": 1}, ["y0 L=256 tile=32x256 col pow2", "y1 L=256 tile=16x256 col pow2"]),
+    (16, 131072, "16", "256,512", {}, ["x0 L=256 tile=16x256 col tma stages=2 ctas=512 smem=98304 B/pt=12",
+                                      "x0 L=256 tile=32x256 col tma stages=2 ctas=256 smem=196608 B/pt=16 [x-inv,grad]",
+                                      "x1 L=512 tile=8x512 row pow2"]),
+    (6144, 128, "384,16", "128", {}, ["y0 L=384 tile=32x384 col tma stages=2", "x0 L=128 tile=32x128 row pow2"]),
+    (6144, 128, "384,16", "128", {"no_tma": 1}, ["y0 L=384 tile=32x384 col pow2"]),
+    (64, 8192, "64", "8192", {}, ["x0 L=8192 tile=1x8192 row pow2", "y0 L=64 tile=16x64 col tma stages=3"]),
+    (64, 8192, "64", "8192", {"tma_nb": 32, "tma_stages": 3}, ["y0 L=64 tile=32x64 col tma stages=3"]),
 ])
-def test_plan_routes_digits_to_the_specialised_kernels(ny, nx, yd, xd, expect):
-    """dop_plan_describe names, per pass, the tile shape and the kernel family the plan chose."""
+def test_plan_routes_digits_to_the_specialised_kernels(ny, nx, yd, xd, tun, expect):
+    """dop_plan_describe names, per pass, the tile shape and the kernel family the plan chose: column passes
+    go to the persistent TMA pipeline (tma_col.cuh) unless dop_tuning.no_tma asks for the LDG/STG kernels."""
     h, _ = dop.dop_plan_create(ny, nx, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0,
-                               tuning=dop.make_tuning(xdigits=_digits(xd), ydigits=_digits(yd), no_cluster=1))
+                               tuning=dop.make_tuning(xdigits=_digits(xd), ydigits=_digits(yd), no_cluster=1, **tun))
     text = dop.dop_plan_describe(h)
     dop.dop_plan_destroy(h)
     for e in expect:
@@ -224,9 +230,10 @@ def test_tuning_is_validated(tun, status):
 def test_loss_scratch_matches_the_launched_loss_pass():
     """ADVICE r1 (medium): with a forced column bundle width the loss pass launches fewer, wider CTAs;
     the scratch and the final reduce must count the CTAs actually launched."""
-    for nb, ctas in ((0, 512), (32, 256), (64, 128)):
+    for tun, ctas in ((dict(no_tma=1), 512), (dict(no_tma=1, col_nb=32), 256), (dict(no_tma=1, col_nb=64), 128),
+                      (dict(), 512), (dict(tma_nb=32), 256)):
         h, _ = dop.dop_plan_create(64, 16384, 0.25e-6, (550e-9,), (1.5,), 1e-3, dop.DOP_LOSS_L2, 0.0, 0,
-                                   tuning=dop.make_tuning(xdigits=(128, 128), col_nb=nb, no_cluster=1))
+                                   tuning=dop.make_tuning(xdigits=(128, 128), no_cluster=1, **tun))
         text = dop.dop_plan_describe(h)
         dop.dop_plan_destroy(h)
         line = [l for l in text.splitlines() if "loss,seed" in l][0]

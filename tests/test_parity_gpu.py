@@ -152,17 +152,37 @@ KERNEL_FAMILIES = [
 ]
 
 
-@pytest.mark.parametrize("generic", [0, 1])
+@pytest.mark.parametrize("family", ["tma", "ldg", "generic"])
 @pytest.mark.parametrize("ny,nx,yd,xd", KERNEL_FAMILIES)
-def test_every_kernel_family_against_the_oracle(ny, nx, yd, xd, generic):
-    """Forces digit decompositions so that each instantiated digit length of the register-blocked
-    kernels (column tile / H / per-lane variants, staged and unstaged row tiles, 3 x 2^k) runs the
-    fused L2 path and is compared with the oracle; generic = 1 runs the same plans on the generic
-    shared-memory kernel (force_generic), i.e. that kernel at full digit lengths."""
+def test_every_kernel_family_against_the_oracle(ny, nx, yd, xd, family):
+    """Forces digit decompositions so that each instantiated digit length of every kernel family runs the
+    fused L2 path and is compared with the oracle: "tma" = the default routing (column passes through the
+    persistent TMA pipeline, tma_col.cuh), "ldg" = the register-blocked LDG/STG kernels alone
+    (dop_tuning.no_tma: column tile / H / per-lane variants, staged and unstaged row tiles, 3 x 2^k),
+    "generic" = the same plans on the generic shared-memory kernel at full digit lengths."""
     cfg = synth.CONFIGS["C4"].scaled(ny, nx)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
-    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(xdigits=digits(xd), ydigits=digits(yd), force_generic=generic,
-                                                      no_cluster=1))
+    tun = dop.make_tuning(xdigits=digits(xd), ydigits=digits(yd), force_generic=int(family == "generic"),
+                          no_tma=int(family == "ldg"), no_cluster=1)
+    I, L, g = run_l2(cfg, h, T, tuning=tun)
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
+@pytest.mark.parametrize("tun", [
+    dict(no_tma=1, col_nb=32), dict(no_tma=1, col_nb=64), dict(tma_nb=32), dict(tma_nb=16, tma_stages=3),
+    dict(no_tma=1, prefetch_waves=-1), dict(no_tma=1, prefetch_waves=3), dict(force_generic=1, tile_pts=1024),
+    dict(force_generic=1, tile_pts=16384), dict(slab_mb=1, slab_streams=3),
+])
+def test_tuning_knobs_only_change_the_rounding_order(tun):
+    """include/dop.h: no dop_tuning field changes a result beyond rounding order.  Every knob on a grid with two
+    x digits and two y digits (the L2 loss pass is then a column-type pass whose CTA count follows the bundle
+    width: the loss partials must match what is launched), against the oracle."""
+    cfg = synth.CONFIGS["C4"].scaled(4096, 16384)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(xdigits=(128, 128), ydigits=(64, 64), no_cluster=1, **tun))
     Ir, Lr, gr = oracle_l2(cfg, h, T)
     check(I, Ir, "intensity")
     check(g, gr, "dL/dh")
