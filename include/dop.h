@@ -58,7 +58,7 @@ typedef enum {
     DOP_OK = 0,
     DOP_ERR_INVALID_ARG = 1,      /* NULL where a pointer is required, non-finite / non-positive
                                      pitch or lambda, n_lambda < 1, bad enum, missing buffer     */
-    DOP_ERR_UNSUPPORTED_SIZE = 2, /* ny or nx < 2, or not of the form 2^a 3^b                    */
+    DOP_ERR_UNSUPPORTED_SIZE = 2, /* ny or nx < 2, or with a prime factor above 127              */
     DOP_ERR_WORKSPACE = 3,        /* NULL workspace                                              */
     DOP_ERR_STATE = 4,            /* adj called before fwd                                       */
     DOP_ERR_ARCH = 5,             /* current device is not compute capability 10.x (sm_100)      */
@@ -117,7 +117,10 @@ typedef struct {
 } dop_tuning;
 
 typedef struct {
-    int64_t ny, nx;            /* rows, columns; x contiguous; each 2^a 3^b, >= 2               */
+    int64_t ny, nx;            /* rows, columns; x contiguous; each >= 2, prime factors <= 127:  */
+                               /* 2^a 3^b run on the specialised kernels, other factors (the     */
+                               /* paper's 28 800 = 2^7 3^2 5^2, 40 000 = 2^6 5^4, 128 640 =      */
+                               /* 2^7 3 5 67) as direct odd-prime butterflies  */
     double pitch;              /* metres, same in x and y                                        */
     int32_t n_lambda;          /* >= 1                                                           */
     const double* lambda;      /* [n_lambda] metres, HOST memory, copied by dop_plan_create      */

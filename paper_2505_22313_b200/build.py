@@ -23,7 +23,7 @@ POW2_INST = [(1, L) for L in (16, 32, 64, 128, 256, 512)] + \
             [(0, L) for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192)]
 POW2_X3 = (16, 32, 64, 128)  # digits 3 * LP
 # (digit length, bundle width, pipeline depth) of the TMA column kernels -- must match DOP_TMA_LIST in kernels_pow2.cu
-TMA_INST = [(64, 32, 3), (64, 16, 3), (128, 32, 3), (128, 16, 3), (256, 32, 2), (256, 16, 3), (256, 16, 2), (512, 16, 2),
+TMA_INST = [(16, 32, 3), (32, 32, 3), (64, 32, 3), (64, 16, 3), (128, 32, 3), (128, 16, 3), (256, 32, 2), (256, 16, 3), (256, 16, 2), (512, 16, 2),
             (96, 32, 3), (192, 32, 3), (384, 32, 2)]
 CLUSTER_INST = [(4096, 2), (4096, 1), (2048, 4), (1024, 8)]  # (local transform length M, lines per CTA S): rows of 16 M
 HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", "cluster_row.cuh", "tma_col.cuh", os.path.join("..", "..", "include", "dop.h")]

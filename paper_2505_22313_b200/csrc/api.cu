@@ -570,7 +570,7 @@ const char* dop_status_string(dop_status s)
     switch (s) {
     case DOP_OK: return "DOP_OK";
     case DOP_ERR_INVALID_ARG: return "DOP_ERR_INVALID_ARG: bad or missing argument";
-    case DOP_ERR_UNSUPPORTED_SIZE: return "DOP_ERR_UNSUPPORTED_SIZE: ny and nx must be 2^a 3^b, >= 2";
+    case DOP_ERR_UNSUPPORTED_SIZE: return "DOP_ERR_UNSUPPORTED_SIZE: ny and nx must be >= 2 with no prime factor above 127";
     case DOP_ERR_WORKSPACE: return "DOP_ERR_WORKSPACE: workspace missing";
     case DOP_ERR_STATE: return "DOP_ERR_STATE: dop_propagate_adj needs a preceding dop_propagate_fwd";
     case DOP_ERR_ARCH: return "DOP_ERR_ARCH: device is not sm_100";

@@ -1,6 +1,6 @@
-// kernels_generic.cu -- the generic tile-pass kernel: any digit length 2^a 3^b, any tile shape,
-// every fused pointwise op.  One CTA = one tile held in shared memory; in-place mixed-radix
-// (2/3/4) decimation-in-frequency forward, mirrored decimation-in-time inverse.
+// kernels_generic.cu -- the generic tile-pass kernel: any digit length whose prime factors are <= 127, any
+// tile shape, every fused pointwise op.  One CTA = one tile held in shared memory; in-place mixed-radix
+// (2/3/4, and direct odd-prime butterflies) decimation-in-frequency forward, mirrored decimation-in-time inverse.
 // It is the correctness backbone and the fallback for shapes the specialised kernels
 // (kernels_pow2.cu) do not cover.
 //
@@ -59,10 +59,120 @@ __device__ __forceinline__ void bfly4(float2* v)
     if (DIR > 0) { v[1] = m; v[3] = q; } else { v[1] = q; v[3] = m; }
 }
 
+// radix-5 / radix-7 butterflies in registers: the same symmetric form as prime_step below, unrolled
+// (cos / sin of 2 pi k / r as constants).  DIR = +1: exp(-2 pi i pc/r).
+template <int DIR>
+__device__ __forceinline__ void bfly5(float2* v)
+{
+    const float c1 = 0.30901699437494742410f, c2 = -0.80901699437494742410f; // cos(2 pi/5), cos(4 pi/5)
+    const float s1 = 0.95105651629515357212f, s2 = 0.58778525229247312917f;  // sin(2 pi/5), sin(4 pi/5)
+    const float2 a1 = cadd(v[1], v[4]), b1 = csub(v[1], v[4]), a2 = cadd(v[2], v[3]), b2 = csub(v[2], v[3]);
+    const float2 x0 = v[0];
+    v[0] = cadd(x0, cadd(a1, a2));
+    const float2 A1 = make_float2(x0.x + c1 * a1.x + c2 * a2.x, x0.y + c1 * a1.y + c2 * a2.y);
+    const float2 A2 = make_float2(x0.x + c2 * a1.x + c1 * a2.x, x0.y + c2 * a1.y + c1 * a2.y);
+    const float2 B1 = make_float2(s1 * b1.x + s2 * b2.x, s1 * b1.y + s2 * b2.y);
+    const float2 B2 = make_float2(s2 * b1.x - s1 * b2.x, s2 * b1.y - s1 * b2.y);
+    // forward: y_k = A_k - i B_k, y_{5-k} = A_k + i B_k
+    const float2 m1 = make_float2(A1.x + B1.y, A1.y - B1.x), q1 = make_float2(A1.x - B1.y, A1.y + B1.x);
+    const float2 m2 = make_float2(A2.x + B2.y, A2.y - B2.x), q2 = make_float2(A2.x - B2.y, A2.y + B2.x);
+    if (DIR > 0) { v[1] = m1; v[4] = q1; v[2] = m2; v[3] = q2; }
+    else { v[1] = q1; v[4] = m1; v[2] = q2; v[3] = m2; }
+}
+template <int DIR>
+__device__ __forceinline__ void bfly7(float2* v)
+{
+    const float c1 = 0.62348980185873353053f, c2 = -0.22252093395631440429f, c3 = -0.90096886790241912624f;
+    const float s1 = 0.78183148246802980871f, s2 = 0.97492791218182360702f, s3 = 0.43388373911755812048f;
+    const float2 a1 = cadd(v[1], v[6]), b1 = csub(v[1], v[6]), a2 = cadd(v[2], v[5]), b2 = csub(v[2], v[5]);
+    const float2 a3 = cadd(v[3], v[4]), b3 = csub(v[3], v[4]);
+    const float2 x0 = v[0];
+    v[0] = cadd(x0, cadd(a1, cadd(a2, a3)));
+    // cos(2 pi c k/7): k=1: c1 c2 c3; k=2: c2 c3 c1; k=3: c3 c1 c2.  sin: k=1: s1 s2 s3; k=2: s2 -s3 -s1; k=3: s3 -s1 s2
+    const float2 A1 = make_float2(x0.x + c1 * a1.x + c2 * a2.x + c3 * a3.x, x0.y + c1 * a1.y + c2 * a2.y + c3 * a3.y);
+    const float2 A2 = make_float2(x0.x + c2 * a1.x + c3 * a2.x + c1 * a3.x, x0.y + c2 * a1.y + c3 * a2.y + c1 * a3.y);
+    const float2 A3 = make_float2(x0.x + c3 * a1.x + c1 * a2.x + c2 * a3.x, x0.y + c3 * a1.y + c1 * a2.y + c2 * a3.y);
+    const float2 B1 = make_float2(s1 * b1.x + s2 * b2.x + s3 * b3.x, s1 * b1.y + s2 * b2.y + s3 * b3.y);
+    const float2 B2 = make_float2(s2 * b1.x - s3 * b2.x - s1 * b3.x, s2 * b1.y - s3 * b2.y - s1 * b3.y);
+    const float2 B3 = make_float2(s3 * b1.x - s1 * b2.x + s2 * b3.x, s3 * b1.y - s1 * b2.y + s2 * b3.y);
+    const float2 m1 = make_float2(A1.x + B1.y, A1.y - B1.x), q1 = make_float2(A1.x - B1.y, A1.y + B1.x);
+    const float2 m2 = make_float2(A2.x + B2.y, A2.y - B2.x), q2 = make_float2(A2.x - B2.y, A2.y + B2.x);
+    const float2 m3 = make_float2(A3.x + B3.y, A3.y - B3.x), q3 = make_float2(A3.x - B3.y, A3.y + B3.x);
+    if (DIR > 0) { v[1] = m1; v[6] = q1; v[2] = m2; v[5] = q2; v[3] = m3; v[4] = q3; }
+    else { v[1] = q1; v[6] = m1; v[2] = q2; v[5] = m2; v[3] = q3; v[4] = m3; }
+}
+
+// One radix-r step for an odd prime r > 3 (the paper's own grids carry 5^2, 5^4 and 67: Table 2):
+// the r-point DFT of every butterfly written out directly, with the conjugate symmetry of its kernel halving the
+// multiplies.  With a_c = x_c + x_{r-c}, b_c = x_c - x_{r-c} (c = 1 .. (r-1)/2):
+//   A_k = sum_c a_c cos(2 pi c k / r),  B_k = sum_c b_c sin(2 pi c k / r),
+//   forward:  y_k = x_0 + A_k - i B_k,  y_{r-k} = x_0 + A_k + i B_k      (inverse: the two swapped).
+// One work item = one output pair (k, r - k) of one butterfly (k = 0: the plain sum); the step runs out of place
+// into the second half of the tile's shared memory (s2) and is copied back, the twiddles W_{n_q}^{j k} ride on
+// the outputs (forward) or are applied to the inputs in a pass of their own (inverse), as in the radix-2/3/4 steps.
+template <int DIR, bool COL>
+__device__ void prime_step(float2* s, float2* s2, const PassDesc& p, int nl_eff, int sl, int se, int r, int nq)
+{
+    const int L = p.L;
+    const float2* __restrict__ wL = p.wL;
+    const int m = nq / r, tws = L / nq, twr = L / r, per_line = L / r, h = (r - 1) / 2;
+    const int total = nl_eff * L;
+    if (DIR < 0 && m > 1) {
+        for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+            int l, i;
+            if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+            const int pos = i % nq, c = pos / m, j = pos - c * m;
+            if (c > 0 && j > 0) s[l * sl + i * se] = cmulc(s[l * sl + i * se], __ldg(wL + j * c * tws));
+        }
+        __syncthreads();
+    }
+    const int items = nl_eff * per_line * (h + 1);
+    for (int it = threadIdx.x; it < items; it += blockDim.x) {
+        int l, jj, kk;
+        if (COL) { l = it % nl_eff; const int rest = it / nl_eff; jj = rest % per_line; kk = rest / per_line; }
+        else { jj = it % per_line; const int rest = it / per_line; l = rest % nl_eff; kk = rest / nl_eff; }
+        const int b = jj / m, j = jj - b * m;
+        const int base = l * sl + (b * nq + j) * se, step = m * se;
+        const float2 x0 = s[base];
+        if (kk == 0) {
+            float2 acc = x0;
+            for (int c = 1; c < r; ++c) acc = cadd(acc, s[base + c * step]);
+            s2[base] = acc;
+        } else {
+            float2 A = make_float2(0.0f, 0.0f), B = make_float2(0.0f, 0.0f);
+            int q = 0;
+            for (int c = 1; c <= h; ++c) {
+                q += kk;
+                if (q >= r) q -= r;
+                const float2 w = __ldg(wL + q * twr); // (cos, -sin) of 2 pi c k / r
+                const float2 xa = s[base + c * step], xb = s[base + (r - c) * step];
+                const float2 sum = cadd(xa, xb), dif = csub(xa, xb);
+                A.x = fmaf(sum.x, w.x, A.x);
+                A.y = fmaf(sum.y, w.x, A.y);
+                B.x = fmaf(dif.x, -w.y, B.x);
+                B.y = fmaf(dif.y, -w.y, B.y);
+            }
+            const float2 t = cadd(x0, A);
+            const float2 iB = make_float2(-B.y, B.x);
+            float2 yk = DIR > 0 ? csub(t, iB) : cadd(t, iB);
+            float2 yr = DIR > 0 ? cadd(t, iB) : csub(t, iB);
+            if (DIR > 0 && j > 0) {
+                yk = cmul(yk, __ldg(wL + j * kk * tws));
+                yr = cmul(yr, __ldg(wL + j * (r - kk) * tws));
+            }
+            s2[base + kk * step] = yk;
+            s2[base + (r - kk) * step] = yr;
+        }
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < total; idx += blockDim.x) s[idx] = s2[idx];
+    __syncthreads();
+}
+
 // In-place L-point DFT on every line of the tile in shared memory.
 // Element (line l, slot i) lives at s[l*sl + i*se].
 template <int DIR, bool COL>
-__device__ void tile_fft(float2* s, const PassDesc& p, int nl_eff, int sl, int se)
+__device__ void tile_fft(float2* s, float2* s2, const PassDesc& p, int nl_eff, int sl, int se)
 {
     const int L = p.L;
     const float2* __restrict__ wL = p.wL;
@@ -71,6 +181,11 @@ __device__ void tile_fft(float2* s, const PassDesc& p, int nl_eff, int sl, int s
         const int q = (DIR > 0) ? qq : (p.n_radix - 1 - qq);
         const int r = p.radix[q];
         if (DIR < 0) nq *= r;       // inverse walks the steps backwards: n_q grows
+        if (r > 7) { // larger odd prime factor: direct r-point butterflies, out of place
+            prime_step<DIR, COL>(s, s2, p, nl_eff, sl, se, r, nq);
+            if (DIR > 0) nq /= r;
+            continue;
+        }
         const int m = nq / r;       // butterfly stride (slots)
         const int tws = L / nq;     // W_{n_q}^x = wL[x * tws]
         const int per_line = L / r;
@@ -81,25 +196,27 @@ __device__ void tile_fft(float2* s, const PassDesc& p, int nl_eff, int sl, int s
             const int b = jj / m, j = jj - b * m;
             float2* e = s + l * sl + (b * nq + j) * se;
             const int step = m * se;
-            float2 v[4];
+            float2 v[7];
 #pragma unroll
-            for (int c = 0; c < 4; ++c)
+            for (int c = 0; c < 7; ++c)
                 if (c < r) v[c] = e[c * step];
             if (DIR < 0) { // DIT mirror: conj twiddle first
 #pragma unroll
-                for (int c = 1; c < 4; ++c)
+                for (int c = 1; c < 7; ++c)
                     if (c < r) v[c] = cmulc(v[c], __ldg(wL + j * c * tws));
             }
             if (r == 4) bfly4<DIR>(v);
             else if (r == 2) bfly2<DIR>(v);
-            else bfly3<DIR>(v);
+            else if (r == 3) bfly3<DIR>(v);
+            else if (r == 5) bfly5<DIR>(v);
+            else bfly7<DIR>(v);
             if (DIR > 0) {
 #pragma unroll
-                for (int c = 1; c < 4; ++c)
+                for (int c = 1; c < 7; ++c)
                     if (c < r) v[c] = cmul(v[c], __ldg(wL + j * c * tws));
             }
 #pragma unroll
-            for (int c = 0; c < 4; ++c)
+            for (int c = 0; c < 7; ++c)
                 if (c < r) e[c * step] = v[c];
         }
         __syncthreads();
@@ -141,6 +258,7 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
     const int se = COL ? nl_eff : 1;
     const long long ls = p.SCc, es = p.es;
     const int total = nl_eff * L;
+    float2* s2 = s + p.nl * L; // scratch of the prime-radix steps (the plan doubles smem_bytes for such digits)
     const long long r0 = p.r_from ? m : c0; // boundary-twiddle r of line 0 (x digit: r = c)
     const int r_per_line = p.r_from ? 0 : 1;
 
@@ -174,8 +292,8 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
     }
     __syncthreads();
 
-    if (p.fft1_dir > 0) tile_fft<1, COL>(s, p, nl_eff, sl, se);
-    else tile_fft<-1, COL>(s, p, nl_eff, sl, se);
+    if (p.fft1_dir > 0) tile_fft<1, COL>(s, s2, p, nl_eff, sl, se);
+    else tile_fft<-1, COL>(s, s2, p, nl_eff, sl, se);
 
     // ---- middle op
     if (p.mid_op == MID_H || p.mid_op == MID_HCONJ || p.mid_op == MID_GAUSS) {
@@ -234,8 +352,8 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
 
     int last_dir = p.fft1_dir;
     if (p.fft2_dir != 0) {
-        if (p.fft2_dir > 0) tile_fft<1, COL>(s, p, nl_eff, sl, se);
-        else tile_fft<-1, COL>(s, p, nl_eff, sl, se);
+        if (p.fft2_dir > 0) tile_fft<1, COL>(s, s2, p, nl_eff, sl, se);
+        else tile_fft<-1, COL>(s, s2, p, nl_eff, sl, se);
         last_dir = p.fft2_dir;
     }
 

@@ -26,7 +26,7 @@ extern template cudaError_t launch_x3<128>(const PassDesc&, int, int, cudaStream
 // TMA column kernels (tma_col.cuh): (digit length, bundle width, pipeline depth) instantiated in the tma_inst.cu
 // objects -- the same list as TMA_INST in build.py
 #define DOP_TMA_LIST(X) \
-    X(64, 32, 3) X(64, 16, 3) X(128, 32, 3) X(128, 16, 3) X(256, 32, 2) X(256, 16, 3) X(256, 16, 2) X(512, 16, 2) \
+    X(16, 32, 3) X(32, 32, 3) X(64, 32, 3) X(64, 16, 3) X(128, 32, 3) X(128, 16, 3) X(256, 32, 2) X(256, 16, 3) X(256, 16, 2) X(512, 16, 2) \
     X(96, 32, 3) X(192, 32, 3) X(384, 32, 2)
 #define DOP_TMA_DECL(L, NB, NST) extern template cudaError_t launch_tma<L, NB, NST>(const PassDesc&, int, int, cudaStream_t);
 DOP_TMA_LIST(DOP_TMA_DECL)

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <functional>
 #include <sstream>
 
 #include "dop_internal.h"
@@ -11,6 +12,19 @@
 namespace dop {
 
 static const long double kPiL = 3.141592653589793238462643383279502884L;
+
+constexpr int kMaxPrime = 127; // largest prime factor a digit may carry (direct butterfly in the generic kernel)
+
+static std::vector<long long> prime_factors(long long n) // with multiplicity, ascending; empty if a factor > kMaxPrime
+{
+    std::vector<long long> f;
+    for (long long q = 2; q <= kMaxPrime && n > 1; ++q)
+        while (n % q == 0) { f.push_back(q); n /= q; }
+    if (n != 1) f.clear();
+    return f;
+}
+
+static bool supported_size(long long n) { return n >= 2 && !prime_factors(n).empty(); }
 
 static bool is_23_smooth(long long n)
 {
@@ -20,10 +34,12 @@ static bool is_23_smooth(long long n)
     return n == 1;
 }
 
-// radix steps for one digit: 3s first, then 4s, then one 2 if needed
+// radix steps for one digit: odd primes > 3 first (largest first), then 3s, then 4s, then one 2 if needed
 static std::vector<int> radix_steps(long long L)
 {
     std::vector<int> r;
+    for (long long q = kMaxPrime; q >= 5; --q)
+        while (L % q == 0 && prime_factors(q).size() == 1) { r.push_back((int)q); L /= q; }
     while (L % 3 == 0) { r.push_back(3); L /= 3; }
     while (L % 4 == 0) { r.push_back(4); L /= 4; }
     if (L % 2 == 0) { r.push_back(2); L /= 2; }
@@ -63,7 +79,7 @@ static std::vector<float2> twiddle_table(long long n)
 // <= lmax_last, as balanced as possible.  A forced decomposition (dop_tuning) overrides; it must
 // multiply to N and respect the same limits.
 static bool split_digits(long long N, long long lmax_first, long long lmax_last, int n_forced,
-                         const int64_t* forced, std::vector<long long>* out)
+                         const int64_t* forced, std::vector<long long>* out, bool last_is_row)
 {
     out->clear();
     if (n_forced > 0) {
@@ -79,11 +95,65 @@ static bool split_digits(long long N, long long lmax_first, long long lmax_last,
     }
     if (N <= lmax_last) { out->push_back(N); return true; }
     // divisors of N
-    std::vector<long long> divs;
-    for (long long a = 1; a <= N; a *= 2)
-        for (long long b = a; b <= N; b *= 3)
-            if (N % b == 0) divs.push_back(b);
+    std::vector<long long> divs{1};
+    {
+        const std::vector<long long> pf = prime_factors(N);
+        for (size_t i = 0; i < pf.size();) {
+            size_t j = i;
+            while (j < pf.size() && pf[j] == pf[i]) ++j;
+            const size_t base = divs.size();
+            long long pw = 1;
+            for (size_t e = i; e < j; ++e) {
+                pw *= pf[i];
+                for (size_t k = 0; k < base; ++k) divs.push_back(divs[k] * pw);
+            }
+            i = j;
+        }
+    }
     std::sort(divs.begin(), divs.end());
+    if (!is_23_smooth(N)) {
+        // General sizes: a digit the register-blocked / TMA kernels handle costs 1, a digit of the generic kernel
+        // 4 plus its largest prime factor / 8 (direct butterflies); the cheapest decomposition into at most four
+        // digits wins, ties go to the smaller largest digit.
+        // The first x digit carries the fused exp(i Phi) / loss / dL/dh ops and the last y digit the (x) H
+        // sandwich: only pure powers of two run those on the specialised kernels (3 * 2^k digits: plain passes).
+        auto digit_cost = [&](long long dgt, bool first, bool last) {
+            const bool col = !(last && last_is_row);
+            const bool fused = last_is_row ? first : last;
+            // (fused x passes stage their fp32 planes by TMA: the line count N / dgt must be a multiple of 4)
+            const bool planes_ok = !(last_is_row && first && !last) || (N / dgt) % 4 == 0;
+            if (pow2_supported(dgt, col) && !(fused && dgt % 3 == 0) && planes_ok) return 1.0;
+            const std::vector<long long> f = prime_factors(dgt);
+            return (fused ? 6.0 : 4.0) + (f.back() > 7 ? (double)f.back() / 4.0 : 0.0);
+        };
+        double best_c = -1.0;
+        long long best_m = 0;
+        std::vector<long long> cur, bestv;
+        std::function<void(long long, double, long long)> rec = [&](long long rem, double cost, long long mx) {
+            if (best_c >= 0.0 && cost >= best_c + 1e-9 && !(cost <= best_c + 1e-9 && mx < best_m)) return;
+            if (rem >= 2 && rem <= lmax_last) { // close with `rem` as the last digit
+                const double c = cost + digit_cost(rem, cur.empty(), true);
+                const long long m2 = std::max(mx, rem);
+                if (best_c < 0.0 || c < best_c - 1e-9 || (c <= best_c + 1e-9 && m2 < best_m)) {
+                    best_c = c; best_m = m2; bestv = cur; bestv.push_back(rem);
+                }
+            }
+            if (cur.size() >= 3) return;
+            for (long long d0 : divs) {
+                // (generic column digits: 16 lines x d0 points, twice that with an out-of-place prime step, in 200 KiB)
+                const std::vector<long long> f0 = prime_factors(d0);
+                const long long lim = (!f0.empty() && f0.back() > 7) ? 512 : 1024;
+                if (d0 < 2 || d0 > std::max(lmax_first, lim) || d0 > lim || rem % d0 != 0 || rem / d0 < 2) continue;
+                cur.push_back(d0);
+                rec(rem / d0, cost + digit_cost(d0, cur.size() == 1, false), std::max(mx, d0));
+                cur.pop_back();
+            }
+        };
+        rec(N, 0.0, 0);
+        if (best_c < 0.0) return false;
+        *out = bestv;
+        return true;
+    }
     // two digits
     long long best = -1, best_cost = 0;
     for (long long d0 : divs) {
@@ -119,6 +189,7 @@ static int wl_table_index(dop_plan* p, long long L)
 
 static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long long>& Ls)
 {
+    const bool tu_no_tma = p->tune.no_tma != 0;
     Axis& ax = p->ax[a];
     ax.N = N;
     ax.dig.resize(Ls.size());
@@ -137,7 +208,10 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         // column-type unless it is the last x digit
         const bool col_type = !(a == 0 && d.st == 1);
         const long long lines = col_type ? (a == 0 ? d.st : p->desc.nx) : p->desc.ny * (N / d.L);
-        d.fast = !p->force_generic && pow2_supported(d.L, col_type) && lines % (col_type ? 16 : pow2_lines(d.L, false)) == 0;
+        // (a column digit whose line count is not a multiple of 16 still counts as fast: the TMA kernels clip ragged
+        // tiles in hardware; the LDG/STG kernels decline such a pass at dispatch and the generic kernel runs it)
+        d.fast = !p->force_generic && pow2_supported(d.L, col_type) &&
+                 (col_type ? (lines % 16 == 0 || !tu_no_tma) : lines % pow2_lines(d.L, false) == 0);
         if (d.fast) d.twg = pow2_group_twiddles(d.L);
         if (d.fast && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
             const long long Nj = d.L * d.st;
@@ -289,6 +363,8 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
     }
     d->n_cgroups = (d->NC + d->nl - 1) / d->nl;
     d->smem_bytes = (int)((long long)d->nl * L * (long long)sizeof(float2));
+    for (int rr : g.radix)
+        if (rr > 7) { d->smem_bytes *= 2; break; } // out-of-place scratch of the larger odd-prime steps (kernels_generic.cu)
     d->threads = 256;
 }
 
@@ -345,7 +421,10 @@ void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow
             if (p->tma_nb) nb = p->tma_nb;
             if (p->tma_stages) nst = p->tma_stages;
             auto fits = [&](int b, int n) {
-                return tma_instantiated(g.L, b, n) && d->NC % b == 0 &&
+                // (TMA global strides are multiples of 16 bytes: complex64 field and, for the fused x variants, fp32 planes)
+                const long long sa = has_plane ? 4 : 2;
+                if (d->es % sa != 0 || (d->n_m > 1 && d->SM % sa != 0) || (d->n_o > 1 && d->SO % sa != 0)) return false;
+                return tma_instantiated(g.L, b, n) && d->NC >= b &&
                        (long long)n * g.L * b * (has_plane ? 12 : 8) <= 227 * 1024 - 2048;
             };
             if (!fits(nb, nst)) { // nearest instantiated choice
@@ -358,7 +437,7 @@ void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow
             if (nst > 0) {
                 d->tma = nst;
                 d->nl = nb;
-                d->n_cgroups = d->NC / nb;
+                d->n_cgroups = (d->NC + nb - 1) / nb; // (a ragged last tile is clipped by the TMA unit)
                 d->smem_bytes = (int)((long long)nst * g.L * nb * (has_plane ? 12 : 8));
                 d->threads = (int)(nb * (g.L / 16) + 32);
                 return;
@@ -383,7 +462,7 @@ void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow
 dop_status build_plan(dop_plan* p)
 {
     const dop_plan_desc& d = p->desc;
-    if (!is_23_smooth(d.nx) || !is_23_smooth(d.ny)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (!supported_size(d.nx) || !supported_size(d.ny)) return DOP_ERR_UNSUPPORTED_SIZE;
     const dop_tuning& tu = p->tune;
     p->force_generic = tu.force_generic != 0;
     // ---- design-loop options
@@ -431,8 +510,8 @@ dop_status build_plan(dop_plan* p)
                               (tu.cluster_force || d.nx == 16384);
     if (want_cluster && tu.n_xdigits == 0) {
         lx = {16, d.nx / 16}; // rows of 16 M points: one thread-block-cluster pass per transform pair
-    } else if (!split_digits(d.nx, 512, 8192, tu.n_xdigits, tu.xdigits, &lx)) return DOP_ERR_UNSUPPORTED_SIZE;
-    if (!split_digits(d.ny, 512, 512, tu.n_ydigits, tu.ydigits, &ly)) return DOP_ERR_UNSUPPORTED_SIZE;
+    } else if (!split_digits(d.nx, 512, 8192, tu.n_xdigits, tu.xdigits, &lx, true)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (!split_digits(d.ny, 512, 512, tu.n_ydigits, tu.ydigits, &ly, false)) return DOP_ERR_UNSUPPORTED_SIZE;
     if (!build_axis(p, 0, d.nx, lx) || !build_axis(p, 1, d.ny, ly)) return DOP_ERR_UNSUPPORTED_SIZE;
     p->x_cluster = want_cluster && lx.size() == 2 && cluster_supported(lx[0], lx[1]) && p->ax[0].dig[0].fast &&
                    p->ax[0].dig[1].fast;

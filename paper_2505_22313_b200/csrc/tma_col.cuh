@@ -218,7 +218,8 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
         t /= ncg;
         const long long m = t % nm;
         const long long o = (long long)(t / nm) + p.o0;
-        const long long line = cg * NB + col;
+        const long long line0 = cg * NB + col;
+        const long long line = line0 < p.NC ? line0 : p.NC - 1; // ragged last tile: clipped lanes read valid table entries
         float2* B = fbuf(s);
         float* Pl = pbuf(s);
 

@@ -61,7 +61,9 @@ def oracle_l2(cfg, h, T, lambdas=None, n_refr=None):
 # small and medium grids: several tiles, ragged tails, radix 3, one- two- and three-digit axes
 # ------------------------------------------------------------------------------------------------
 SHAPES = [(2, 2), (2, 3), (3, 2), (4, 6), (16, 16), (48, 36), (27, 64), (96, 128), (384, 512), (1024, 768),
-          (1536, 2048), (2048, 1024), (243, 256), (4096, 512), (512, 16384), (18, 20736)]
+          (1536, 2048), (2048, 1024), (243, 256), (4096, 512), (512, 16384), (18, 20736),
+          # general sizes: radix 5 / 7 / 11 / 13 / 67 butterflies, one- and two-digit axes
+          (5, 7), (25, 49), (150, 140), (67, 335), (143, 121), (1340, 640), (2880, 2000), (600, 7000)]
 
 
 @pytest.mark.parametrize("ny,nx", SHAPES)
@@ -89,7 +91,8 @@ def test_field_intensity_and_caller_seeded_adjoint(ny, nx):
     check(grad.cpu().numpy(), gref, "dL/dh")
 
 
-@pytest.mark.parametrize("ny,nx", [(2, 2), (6, 4), (96, 128), (384, 512), (1536, 1024), (512, 6144)])
+@pytest.mark.parametrize("ny,nx", [(2, 2), (6, 4), (96, 128), (384, 512), (1536, 1024), (512, 6144),
+                                   (35, 55), (670, 1280), (900, 3600)])
 def test_fused_l2_loss_path(ny, nx):
     # C2's blurred-noise recipe degenerates (zero range) on grids smaller than its blur: tiny grids use C1's
     cfg = synth.CONFIGS["C2" if ny * nx >= 4096 else "C1"].scaled(ny, nx)
