@@ -139,6 +139,15 @@ typedef struct {
                                /* sum-pool of dL/dh (deterministic: lanes, then rows)             */
     int32_t layout_dtype;      /* dop_layout_dtype of d_height                                    */
     double layout_step;        /* metres per gray level (U8 / U16 layouts)                        */
+    /* ---- linear (non-circular) propagation (PAPER.md:436 Matsushima & Shimobaba 2009) ---- */
+    int32_t pad;               /* 0 | 1: the circular operator on the given grid (Eq. 3 as it stands);  */
+                               /* 2: the aperture [ny][nx] sits in the corner of a [2 ny][2 nx] window  */
+                               /* of zero amplitude, the window is propagated and cropped back.  All    */
+                               /* caller planes keep their [ny][nx] shape; the workspace holds the      */
+                               /* window; rows known to be zero / discarded are pruned from the x       */
+                               /* passes.  DOP_LOSS_L2 / DOP_LOSS_NONE, no pre-filter, fp32 layout.     */
+    int32_t band_limit;        /* != 0 (needs pad = 2): H is clipped to |fx| <= u_limit, |fy| <= v_limit, */
+                               /* u_limit = 1 / (lambda sqrt((2 du z)^2 + 1)), du = 1 / (2 nx pitch)      */
 } dop_plan_desc;
 
 /* Adam with a cosine learning-rate schedule (Kingma & Ba 2014, Algorithm 1), applied

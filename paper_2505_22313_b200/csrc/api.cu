@@ -77,6 +77,10 @@ dop_status ensure_device(dop_plan* p)
     }
     size_t f2_off[2], g_off[2];
     for (int a = 0; a < 2; ++a) { f2_off[a] = off; off += align256(p->ax[a].f2.size() * sizeof(double)); }
+    std::vector<size_t> bl_off[2];
+    if (p->desc.band_limit)
+        for (int a = 0; a < 2; ++a)
+            for (int l = 0; l < p->desc.n_lambda; ++l) { bl_off[a].push_back(off); off += align256(p->ax[a].f2.size() * sizeof(double)); }
     for (int a = 0; a < 2; ++a) { g_off[a] = off; off += align256(p->ax[a].g.size() * sizeof(float)); }
 
     char* arena = nullptr;
@@ -102,6 +106,18 @@ dop_status ensure_device(dop_plan* p)
         up(f2_off[a], p->ax[a].f2.data(), p->ax[a].f2.size() * sizeof(double));
         up(g_off[a], p->ax[a].g.data(), p->ax[a].g.size() * sizeof(float));
         p->d_f2[a] = (double*)(arena + f2_off[a]);
+        if (p->desc.band_limit) { // H clipped to |f| <= 1 / (lambda sqrt((2 df z)^2 + 1)), df = 1 / (N pitch) of the window
+            p->d_f2_bl[a].clear();
+            for (int l = 0; l < p->desc.n_lambda; ++l) {
+                const double lam = p->lambda[(size_t)l], df = 1.0 / (2.0 * (double)(a == 0 ? p->ap_nx : p->ap_ny) * p->desc.pitch);
+                const double lim = 1.0 / (lam * std::sqrt((2.0 * df * p->desc.z) * (2.0 * df * p->desc.z) + 1.0));
+                std::vector<double> t = p->ax[a].f2;
+                for (size_t sl = 0; sl < t.size(); ++sl)
+                    if (std::fabs(p->ax[a].fsigned[sl]) > lim) t[sl] = 1e300; // a < 0: zeroed like an evanescent bin
+                up(bl_off[a][(size_t)l], t.data(), t.size() * sizeof(double));
+                p->d_f2_bl[a].push_back((double*)(arena + bl_off[a][(size_t)l]));
+            }
+        }
         p->d_g[a] = (float*)(arena + g_off[a]);
     }
     if (!ok) { cudaFree(arena); p->d_arena = nullptr; return DOP_ERR_CUDA; }
@@ -120,7 +136,8 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     // (a cluster pass takes its group twiddles from x digit 1 and its boundary twiddles from x digit 0)
     const Digit& g = p->ax[t.axis].dig[(size_t)(t.cluster ? 1 : t.digit)];
     char* arena = (char*)p->d_arena;
-    const size_t npts = (size_t)p->desc.nx * (size_t)p->desc.ny;
+    const size_t npts = (size_t)p->desc.nx * (size_t)p->desc.ny;                           // field window
+    const size_t nap = p->ap_nx > 0 ? (size_t)p->ap_nx * (size_t)p->ap_ny : npts;          // caller planes
     d.fft1_dir = t.fft1_dir;
     d.fft2_dir = t.fft2_dir;
     d.wL = (const float2*)(arena + p->wl_off[(size_t)g.wl_index]);
@@ -146,7 +163,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.h_step = (float)p->desc.layout_step;
     const bool hl = (t.load_op == LD_HEIGHT || t.store_op == ST_GRAD) && b.height_is_layout;
     if (hl) { d.up_lg = p->up_lg; d.h_dtype = (int)p->desc.layout_dtype; }
-    if (t.load_op == LD_SEED) d.plane_in = b.dLdI + npts * (size_t)lam;
+    if (t.load_op == LD_SEED) d.plane_in = b.dLdI + nap * (size_t)lam;
     if (t.load_op == LD_SEED_SIMSE) {
         d.plane_in = b.target;
         d.coef = (const float*)(ws + p->ws_coef_off) + 4 * (size_t)lam;
@@ -164,7 +181,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
         d.loss_scratch = (double*)(ws + p->ws_loss_off) + 4 * (size_t)p->loss_tiles * (size_t)lam;
         if (p->desc.flags & DOP_WRITE_INTENSITY) {
             d.write_intensity = 1;
-            d.plane_out = b.intensity + npts * (size_t)lam;
+            d.plane_out = b.intensity + nap * (size_t)lam;
         }
     }
     if (t.mid_op == MID_LOSS) {
@@ -172,7 +189,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
         d.loss_scratch = (double*)(ws + p->ws_loss_off) + (size_t)p->loss_tiles * (size_t)lam;
         if (p->desc.flags & DOP_WRITE_INTENSITY) {
             d.write_intensity = 1;
-            d.plane_out = b.intensity + npts * (size_t)lam;
+            d.plane_out = b.intensity + nap * (size_t)lam;
         }
     }
     if (t.store_op == ST_GRAD) {
@@ -186,7 +203,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
             d.adam_eps = b.adam->eps;
         }
     }
-    if (t.store_op == ST_C64_INTENSITY) d.plane_out = b.intensity + npts * (size_t)lam;
+    if (t.store_op == ST_C64_INTENSITY) d.plane_out = b.intensity + nap * (size_t)lam;
     if (t.store_op == ST_REAL) {
         d.plane_out = b.real_dst;
         if (b.real_dst_pool) { d.pool_out = 1; d.up_lg = p->up_lg; }
@@ -195,7 +212,8 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.phase_coef = (float)((n - 1.0) / lambda);
     d.grad_coef = (float)(2.0 * M_PI * (n - 1.0) / lambda);
     d.scale = (float)(1.0 / (double)npts);
-    d.seed_coef = (float)(4.0 / (double)npts);
+    d.seed_coef = (float)(4.0 / (double)nap);
+    if (p->ap_nx > 0 && t.axis == 0) { d.ap_nx = p->ap_nx; d.ap_ny = p->ap_ny; d.grid_nx = p->desc.nx; }
     d.inv_lam2 = 1.0 / (lambda * lambda);
     d.z = p->desc.z;
     d.h_fixed = (std::fabs(p->desc.z) / lambda < 524288.0 && !p->h_float) ? 1 : 0;
@@ -218,6 +236,7 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.device = p->device;
     d.fx2 = p->d_f2[0];
     d.fy2 = p->d_f2[1];
+    if (p->desc.band_limit) { d.fx2 = p->d_f2_bl[0][(size_t)lam]; d.fy2 = p->d_f2_bl[1][(size_t)lam]; }
     d.gx = p->d_g[0];
     d.gy = p->d_g[1];
     return d;
@@ -244,6 +263,17 @@ long long prof_begin(dop_plan* p, const std::string& name, double bpp, cudaStrea
 void prof_end(dop_plan* p, long long slot, cudaStream_t st)
 {
     if (slot >= 0) cudaEventRecord(p->ev_stop[(size_t)slot], st);
+}
+
+// pad = 2: rows [ap_ny, 2 ap_ny) of wavelength lam's window are known zeros (forward) / discarded (adjoint): the x
+// passes are launched on the aperture rows only and those rows are cleared instead (a write, no read, no DFT)
+bool zero_pruned_rows(const dop_plan* p, char* ws, int lam, cudaStream_t st)
+{
+    if (p->ap_nx == 0) return true;
+    const size_t npts = (size_t)p->desc.nx * (size_t)p->desc.ny;
+    char* field = ws + align256(npts * sizeof(float2)) * (size_t)lam;
+    const size_t row = (size_t)p->desc.nx * sizeof(float2);
+    return cudaMemsetAsync(field + (size_t)p->ap_ny * row, 0, (size_t)(p->desc.ny - p->ap_ny) * row, st) == cudaSuccess;
 }
 
 long long gcdll(long long a, long long b) { while (b) { long long t = a % b; a = b; b = t; } return a; }
@@ -387,6 +417,11 @@ dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* works
         if (!std::isfinite(d->n_refr[i])) return DOP_ERR_INVALID_ARG;
     }
     if (d->ny < 2 || d->nx < 2) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (d->pad != 0 && d->pad != 1 && d->pad != 2) return DOP_ERR_INVALID_ARG;
+    if (d->pad == 2 && (d->loss == DOP_LOSS_SIMSE || d->prefilter_sigma_px > 0.0 || (d->upsample != 0 && d->upsample != 1) ||
+                        d->layout_dtype != DOP_LAYOUT_F32))
+        return DOP_ERR_INVALID_ARG;
+    if (d->band_limit != 0 && d->pad != 2) return DOP_ERR_INVALID_ARG;
     dop_plan* p = new (std::nothrow) dop_plan();
     if (p == nullptr) return DOP_ERR_INVALID_ARG;
     p->desc = *d;
@@ -396,6 +431,12 @@ dop_status dop_plan_create(dop_plan** out, const dop_plan_desc* d, size_t* works
     p->desc.n_refr = p->n_refr.data();
     if (d->tuning != nullptr) p->tune = *d->tuning;
     p->desc.tuning = nullptr;
+    if (d->pad == 2) { // the plan is built for the [2 ny][2 nx] window; the caller's planes keep the aperture shape
+        p->ap_ny = d->ny;
+        p->ap_nx = d->nx;
+        p->desc.ny = 2 * d->ny;
+        p->desc.nx = 2 * d->nx;
+    }
     dop_status s;
     try {
         s = build_plan(p);
@@ -439,9 +480,13 @@ dop_status dop_propagate_fwd(dop_plan* p, const void* d_height, const float* d_t
         b.height = heff;
         b.height_is_layout = false;
     }
-    for (int lam = 0; lam < p->desc.n_lambda; ++lam)
+    for (int lam = 0; lam < p->desc.n_lambda; ++lam) {
+        if (!zero_pruned_rows(p, ws, lam, st)) return DOP_ERR_CUDA; // pad = 2: the window rows below the aperture enter as zeros
         if ((s = run(p, p->fwd, lam, b, ws, st, "fwd")) != DOP_OK) return s;
-    const double npts = (double)p->desc.nx * (double)p->desc.ny;
+        // ... and leave the loss pass as a zero seed (DOP_LOSS_L2: the x passes only touch the aperture rows)
+        if (l2 && !zero_pruned_rows(p, ws, lam, st)) return DOP_ERR_CUDA;
+    }
+    const double npts = p->ap_nx > 0 ? (double)p->ap_nx * (double)p->ap_ny : (double)p->desc.nx * (double)p->desc.ny;
     if (l2 && d_loss != nullptr) {
         long long slot = prof_begin(p, "fwd:loss-reduce", 0.0, st);
         cudaError_t e = launch_loss_reduce((const double*)(ws + p->ws_loss_off), p->loss_tiles * p->desc.n_lambda,
@@ -512,8 +557,11 @@ static dop_status propagate_adj(dop_plan* p, const void* d_height, const float* 
         }
     }
     if (p->desc.loss == DOP_LOSS_SIMSE) b.target = p->target_seen;
-    for (int lam = 0; lam < p->desc.n_lambda; ++lam)
+    for (int lam = 0; lam < p->desc.n_lambda; ++lam) {
+        // pad = 2, caller-seeded adjoint: the seed is zero below the aperture rows
+        if (p->desc.loss == DOP_LOSS_NONE && !zero_pruned_rows(p, ws, lam, st)) return DOP_ERR_CUDA;
         if ((s = run(p, p->adj, lam, b, ws, st, "adj")) != DOP_OK) return s;
+    }
     if (has_pre) { // A6: the Gaussian spectrum is real and even, so the filter is self-adjoint
         Buffers pb;
         pb.real_src = b.grad;

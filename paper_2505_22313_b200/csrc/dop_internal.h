@@ -115,6 +115,8 @@ struct PassDesc {
     int threads;
     int cluster;          // 1 (exchange through L2) | 2 (through DSMEM) = cluster row pass (cluster_row.cuh): L = M, the x digits (16, M) fused; n_o rows
     int device;           // the plan's device (function attributes are set once per device)
+    long long ap_nx, ap_ny, grid_nx; // pad = 2 (generic kernel): the caller's planes are [ap_ny][ap_nx], the field window
+                          // has rows of grid_nx points; plane accesses outside the aperture are masked (ap_nx = 0: no padding)
     int tma;              // > 0: TMA column kernel (tma_col.cuh) with this many tiles in flight per CTA; nl = its bundle width
 };
 
@@ -163,6 +165,7 @@ struct Axis {
     std::vector<Digit> dig;
     std::vector<long long> kslot; // slot -> frequency index in [0, N)
     std::vector<double> f2;       // slot -> f^2
+    std::vector<double> fsigned;  // slot -> signed frequency f (band limit)
     std::vector<float> g;         // slot -> Gaussian factor (pre-filter)
 };
 
@@ -205,6 +208,8 @@ struct dop_plan {
     long long loss_tiles = 0;                 // CTAs of the MID_LOSS pass
     size_t ws_fields = 0, ws_heff_off = 0, ws_loss_off = 0, ws_xpool_off = 0, ws_coef_off = 0, ws_gfine_off = 0, ws_bytes = 0;
     int up_lg = 0;              // log2(upsample)
+    long long ap_ny = 0, ap_nx = 0; // pad = 2: the caller's aperture (desc.ny, desc.nx then hold the 2x window); 0 = no padding
+    std::vector<double*> d_f2_bl[2]; // band_limit: per-wavelength f^2 tables with the clipped bins set to 1e300
     // device tables (lazy)
     bool dev_ready = false;
     int device = -1;

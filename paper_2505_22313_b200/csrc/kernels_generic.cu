@@ -236,6 +236,16 @@ __device__ __forceinline__ float layout_height(const PassDesc& p, const void* ba
     return p.h_step * (float)((const unsigned short*)base)[ci];
 }
 
+// pad = 2 (dop_plan_desc.pad): the field offset `off` of a point of the [.][grid_nx] window -> the offset of the same
+// point in the caller's [ap_ny][ap_nx] planes, or -1 outside the aperture (zero amplitude on the way in, nothing to
+// compare or to store on the way out).  ap_nx = 0: no padding, planes and field share their offsets.
+__device__ __forceinline__ long long plane_offset(const PassDesc& p, long long off)
+{
+    if (p.ap_nx == 0) return off;
+    const long long row = off / p.grid_nx, x = off - row * p.grid_nx;
+    return (x < p.ap_nx && row < p.ap_ny) ? row * p.ap_nx + x : -1;
+}
+
 template <bool COL>
 __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
 {
@@ -268,14 +278,17 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
         if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
         const long long off = base + l * ls + i * es;
         float2 v;
+        const long long poff = (p.load_op == LD_HEIGHT || p.load_op == LD_SEED) ? plane_offset(p, off) : off;
         if (p.load_op == LD_C64) {
             v = p.field[off];
+        } else if (poff < 0) {                       // outside the aperture: zero amplitude / zero seed
+            v = make_float2(0.0f, 0.0f);
         } else if (p.load_op == LD_HEIGHT) {
-            float tt = layout_height(p, p.height, off) * p.phase_coef; // Eq. (1) in turns
+            float tt = layout_height(p, p.height, poff) * p.phase_coef; // Eq. (1) in turns
             sincospif(2.0f * tt, &v.y, &v.x);        // Eq. (2), E_in = 1
         } else if (p.load_op == LD_SEED) {
             float2 u = p.field[off];
-            float g = 2.0f * p.plane_in[off];
+            float g = 2.0f * p.plane_in[poff];
             v = make_float2(g * u.x, g * u.y);
         } else if (p.load_op == LD_SEED_SIMSE) {     // Eq. (6): 2 dL/dI = c0 + cI I + cT T
             float2 u = p.field[off];
@@ -331,12 +344,17 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
             if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
             const long long off = base + l * ls + i * es;
             float2 v = s[l * sl + i * se];
+            const long long poff = plane_offset(p, off);
+            if (poff < 0) {                        // outside the aperture: no loss term, zero seed
+                s[l * sl + i * se] = make_float2(0.0f, 0.0f);
+                continue;
+            }
             float I = v.x * v.x + v.y * v.y;      // F6
-            float d = I - p.plane_in[off];         // F7
+            float d = I - p.plane_in[poff];        // F7
             acc += (double)d * (double)d;
             float g = p.seed_coef * d;             // A1: 2 gI = 4 (I - T)/N
             s[l * sl + i * se] = make_float2(g * v.x, g * v.y);
-            if (p.write_intensity) p.plane_out[off] = I;
+            if (p.write_intensity) p.plane_out[poff] = I;
         }
         // deterministic block reduction: warp shuffle tree, then warp 0 over the 8 partials
         for (int d = 16; d > 0; d >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, d);
@@ -367,8 +385,20 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
             long long r = r0 + (long long)l * r_per_line;
             v = cmul(v, __ldg(p.tw_b + r * p.pi[i]));
         }
+        const long long poff = p.store_op == ST_C64 ? off : plane_offset(p, off);
         if (p.store_op == ST_C64) {
             p.field[off] = v;
+        } else if (poff < 0) {                       // outside the aperture: the field is kept, no plane to write
+            if (p.store_op == ST_C64_INTENSITY) p.field[off] = v;
+        } else if (p.ap_nx != 0 && (p.store_op == ST_GRAD || p.store_op == ST_GRAD_ACC)) {
+            float sn, cs;
+            sincospif(2.0f * (p.height[poff] * p.phase_coef), &sn, &cs);
+            float g = p.grad_coef * (cs * v.y - sn * v.x); // A5 on the aperture
+            if (p.store_op == ST_GRAD_ACC) g += p.plane_out[poff];
+            p.plane_out[poff] = g;
+        } else if (p.ap_nx != 0 && p.store_op == ST_C64_INTENSITY) {
+            p.field[off] = v;
+            p.plane_out[poff] = v.x * v.x + v.y * v.y;
         } else if (p.store_op == ST_GRAD || p.store_op == ST_GRAD_ACC) {
             const float hv = layout_height(p, p.height, off);
             float tt = hv * p.phase_coef;

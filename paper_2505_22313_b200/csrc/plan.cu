@@ -212,6 +212,9 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         // tiles in hardware; the LDG/STG kernels decline such a pass at dispatch and the generic kernel runs it)
         d.fast = !p->force_generic && pow2_supported(d.L, col_type) &&
                  (col_type ? (lines % 16 == 0 || !tu_no_tma) : lines % pow2_lines(d.L, false) == 0);
+        // pad = 2: the fused x passes mask their plane accesses to the aperture, which only the generic kernel
+        // implements (the plain x passes and every y pass keep the specialised kernels)
+        if (p->ap_nx > 0 && a == 0 && j == 0) d.fast = false;
         if (d.fast) d.twg = pow2_group_twiddles(d.L);
         if (d.fast && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
             const long long Nj = d.L * d.st;
@@ -226,6 +229,7 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
     // slot -> true frequency index:  k = sum_j pi_j(p_j) (L_0 .. L_{j-1})
     ax.kslot.resize((size_t)N);
     ax.f2.resize((size_t)N);
+    ax.fsigned.resize((size_t)N);
     ax.g.resize((size_t)N);
     const double pitch = p->desc.pitch, sigma = p->desc.prefilter_sigma_px;
     for (long long s = 0; s < N; ++s) {
@@ -240,6 +244,7 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         double kb = (double)(k < (N + 1) / 2 ? k : k - N);
         double f = kb / ((double)N * pitch);
         ax.f2[(size_t)s] = f * f;
+        ax.fsigned[(size_t)s] = f;
         double v = kb / (double)N;
         ax.g[(size_t)s] = (float)std::exp(-2.0 * M_PI * M_PI * sigma * sigma * (v * v));
     }
@@ -372,7 +377,25 @@ void tile_geometry(const dop_plan* p, int axis, int digit, PassDesc* d)
 // is a property of the pass (it does not change where data lives): plain forward / inverse
 // passes (and the exp(i Phi) pass of short digits) take wider bundles (pow2_lines), the register-heavy fused
 // variants stay at 16 columns.
+static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow_tma);
+
+// pad = 2: every x pass runs on the aperture rows only (rows below are known zeros on the way in and discarded on
+// the way out: "pruned" passes); the geometry of the full window is cut down to the first ap_ny rows here, so that
+// describe, the loss partial count and the launches all see the same tiles.
 void pass_geometry(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow_tma)
+{
+    pass_geometry_full(p, t, d, allow_tma);
+    if (p->ap_nx == 0 || t.axis != 0) return;
+    if (d->col_type) {
+        d->n_o = p->ap_ny;
+    } else {
+        const long long lpr = p->desc.nx / d->L; // lines per row
+        d->NC = p->ap_ny * lpr;
+        d->n_cgroups = (d->NC + d->nl - 1) / d->nl;
+    }
+}
+
+static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d, bool allow_tma)
 {
     if (t.cluster) { // one cluster of C CTAs per row; CTA = S lines of M points
         const long long M = p->ax[0].dig[1].L;
@@ -506,7 +529,7 @@ dop_status build_plan(dop_plan* p)
     // 5-15 % against two digit passes for clusters of 4-16 (profiles/r02_cluster.md), so only the
     // former is a default; dop_tuning.cluster_force selects them wherever they exist.
     const bool may_cluster = !tu.no_cluster && !p->force_generic;
-    const bool want_cluster = may_cluster && d.nx % 16 == 0 && cluster_supported(16, d.nx / 16) &&
+    const bool want_cluster = may_cluster && p->ap_nx == 0 && d.nx % 16 == 0 && cluster_supported(16, d.nx / 16) &&
                               (tu.cluster_force || d.nx == 16384);
     if (want_cluster && tu.n_xdigits == 0) {
         lx = {16, d.nx / 16}; // rows of 16 M points: one thread-block-cluster pass per transform pair
@@ -568,7 +591,7 @@ std::string describe_plan(const dop_plan* p)
     os << "grid ny=" << d.ny << " nx=" << d.nx << " n_lambda=" << d.n_lambda
        << " loss=" << (d.loss == DOP_LOSS_L2 ? "L2" : d.loss == DOP_LOSS_SIMSE ? "si-mse+energy" : "none")
        << " upsample=" << (1 << p->up_lg) << " layout=" << (d.layout_dtype == DOP_LAYOUT_U8 ? "u8" : d.layout_dtype == DOP_LAYOUT_U16 ? "u16" : "f32")
-       << " prefilter_sigma_px=" << d.prefilter_sigma_px
+       << " prefilter_sigma_px=" << d.prefilter_sigma_px << " pad=" << (p->ap_nx > 0 ? 2 : 1) << " band_limit=" << (d.band_limit ? 1 : 0)
        << " workspace_bytes=" << p->ws_bytes << " loss_tiles=" << p->loss_tiles << "\n";
     for (int a = 0; a < 2; ++a) {
         os << (a == 0 ? "x" : "y") << "-digits:";

@@ -47,6 +47,7 @@ class dop_plan_desc(C.Structure):
         ("loss", C.c_int), ("prefilter_sigma_px", C.c_double), ("flags", C.c_uint32),
         ("tuning", C.POINTER(dop_tuning)),
         ("energy_beta", C.c_double), ("upsample", C.c_int32), ("layout_dtype", C.c_int32), ("layout_step", C.c_double),
+        ("pad", C.c_int32), ("band_limit", C.c_int32),
     ]
 
 
@@ -130,7 +131,7 @@ def _ptr(t: Optional[torch.Tensor], dtype, what: str) -> Optional[int]:
 def dop_plan_create(ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
                     z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0,
                     tuning: Optional[dop_tuning] = None, energy_beta: float = 0.0, upsample: int = 0,
-                    layout_dtype: int = DOP_LAYOUT_F32, layout_step: float = 0.0):
+                    layout_dtype: int = DOP_LAYOUT_F32, layout_step: float = 0.0, pad: int = 0, band_limit: int = 0):
     """-> (plan handle, workspace_bytes).  Host-only; raises DopError on a bad description."""
     nl = len(lambdas)
     lam = (C.c_double * max(nl, 1))(*[float(v) for v in lambdas])
@@ -138,7 +139,7 @@ def dop_plan_create(ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_
     d = dop_plan_desc(int(ny), int(nx), float(pitch), nl, lam, nr, float(z), int(loss),
                       float(prefilter_sigma_px), int(flags),
                       C.pointer(tuning) if tuning is not None else None,
-                      float(energy_beta), int(upsample), int(layout_dtype), float(layout_step))
+                      float(energy_beta), int(upsample), int(layout_dtype), float(layout_step), int(pad), int(band_limit))
     out, ws = C.c_void_p(), C.c_size_t(0)
     st = _lib.dop_plan_create(C.byref(out), C.byref(d), C.byref(ws))
     if st != DOP_OK:
@@ -222,12 +223,14 @@ class Plan:
     def __init__(self, ny: int, nx: int, pitch: float, lambdas: Sequence[float], n_refr: Sequence[float],
                  z: float, loss: int = DOP_LOSS_L2, prefilter_sigma_px: float = 0.0, flags: int = 0,
                  device: str = "cuda:0", tuning: Optional[dop_tuning] = None, energy_beta: float = 0.0,
-                 upsample: int = 0, layout_dtype: int = DOP_LAYOUT_F32, layout_step: float = 0.0):
+                 upsample: int = 0, layout_dtype: int = DOP_LAYOUT_F32, layout_step: float = 0.0, pad: int = 0,
+                 band_limit: int = 0):
         self.ny, self.nx, self.n_lambda, self.loss, self.flags = int(ny), int(nx), len(lambdas), loss, flags
+        self.pad = 2 if pad == 2 else 1
         self.layout_dtype = layout_dtype
         self.handle, self.workspace_bytes = dop_plan_create(ny, nx, pitch, lambdas, n_refr, z, loss,
                                                             prefilter_sigma_px, flags, tuning, energy_beta, upsample,
-                                                            layout_dtype, layout_step)
+                                                            layout_dtype, layout_step, pad, band_limit)
         self.device = torch.device(device)
         self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
         self.launches = dop_plan_launch_count(self.handle)
@@ -246,13 +249,15 @@ class Plan:
                                self.workspace, stream)
 
     def field(self) -> torch.Tensor:
-        """complex64 view [n_lambda, ny, nx] of the workspace fields (valid after a DOP_LOSS_NONE fwd)."""
-        n = self.ny * self.nx
+        """complex64 view [n_lambda, ny, nx] of the workspace fields (valid after a DOP_LOSS_NONE fwd); with
+        pad = 2 the aperture corner of each [2 ny, 2 nx] window."""
+        wy, wx = self.ny * self.pad, self.nx * self.pad
+        n = wy * wx
         stride = (n * 8 + 255) // 256 * 256
         out = []
         for l in range(self.n_lambda):
-            raw = self.workspace[l * stride: l * stride + n * 8].view(torch.float32).view(self.ny, self.nx, 2)
-            out.append(torch.view_as_complex(raw))
+            raw = self.workspace[l * stride: l * stride + n * 8].view(torch.float32).view(wy, wx, 2)
+            out.append(torch.view_as_complex(raw)[: self.ny, : self.nx])
         return torch.stack(out)
 
     def close(self) -> None:

@@ -261,3 +261,20 @@ def test_the_papers_own_grid_sizes_plan(ny, nx, expect):
     for e in expect:
         assert e in text, (e, text)
     assert ws >= ny * nx * 8
+
+
+def test_pad_and_band_limit_arguments_are_validated():
+    """dop_plan_desc.pad / band_limit: host-side validation and the window-sized workspace."""
+    args = (64, 64, 0.25e-6, (550e-9,), (1.5,), 1e-3)
+    for kw in (dict(pad=3), dict(band_limit=1), dict(pad=2, prefilter_sigma_px=2.0), dict(pad=2, upsample=2),
+               dict(pad=2, loss=dop.DOP_LOSS_SIMSE)):
+        with pytest.raises(dop.DopError) as e:
+            dop.dop_plan_create(*args, **kw)
+        assert e.value.status == dop.DOP_ERR_INVALID_ARG
+    hnd, ws = dop.dop_plan_create(*args, pad=2, band_limit=1)
+    text = dop.dop_plan_describe(hnd)
+    dop.dop_plan_destroy(hnd)
+    assert ws >= 4 * 64 * 64 * 8 and "grid ny=128 nx=128" in text and "pad=2 band_limit=1" in text
+    # the x passes are pruned to the aperture rows: half the CTAs of the full window
+    line = [l for l in text.splitlines() if "h->u0" in l][0]
+    assert "ctas=2 " in line, line   # 64 aperture rows of 128 points = 2 tiles of 32 lines (the window has 128 rows)
