@@ -80,28 +80,29 @@ __host__ __device__ constexpr int tma_min_blocks(int smem, int threads)
 // The register-blocked DFT of fft_regs.cuh run out of a tile buffer that already holds the data in the
 // exchange layout: v enters in the layout of group G (forward) and leaves in the layout of the last
 // group; every group boundary is one store, one barrier among the NCOMP compute threads, one load
-// (a thread only ever overwrites slots it has read itself, so no second barrier is needed).
-template <class TL, class S, int G, int NCOMP>
-__device__ __forceinline__ void fwd_groups(float2* v, float2* B, int tt, int col, const float2* __restrict__ tw)
+// (a thread only ever overwrites slots it has read itself, so no second barrier is needed).  `bar` / NBAR: the named
+// barrier and its thread count (digits 3 LP: each sub-tile's thread group exchanges on a barrier of its own).
+template <class TL, class S, int G, int NBAR>
+__device__ __forceinline__ void fwd_groups(float2* v, float2* B, int tt, int col, const float2* __restrict__ tw, int bar = 1)
 {
     TL::template butterflies<G, +1>(v, tt, tw);
     if constexpr (G + 1 < S::NG) {
         TL::template to_smem<G>(v, B, tt, col);
-        asm volatile("bar.sync 1, %0;" ::"n"(NCOMP) : "memory");
+        asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(NBAR) : "memory");
         TL::template from_smem<G + 1>(v, B, tt, col);
-        fwd_groups<TL, S, G + 1, NCOMP>(v, B, tt, col, tw);
+        fwd_groups<TL, S, G + 1, NBAR>(v, B, tt, col, tw, bar);
     }
 }
 // inverse: v enters in the layout of group G (the last one) and leaves in the layout of group 0
-template <class TL, class S, int G, int NCOMP>
-__device__ __forceinline__ void inv_groups(float2* v, float2* B, int tt, int col, const float2* __restrict__ tw)
+template <class TL, class S, int G, int NBAR>
+__device__ __forceinline__ void inv_groups(float2* v, float2* B, int tt, int col, const float2* __restrict__ tw, int bar = 1)
 {
     TL::template butterflies<G, -1>(v, tt, tw);
     if constexpr (G > 0) {
         TL::template to_smem<G>(v, B, tt, col);
-        asm volatile("bar.sync 1, %0;" ::"n"(NCOMP) : "memory");
+        asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(NBAR) : "memory");
         TL::template from_smem<G - 1>(v, B, tt, col);
-        inv_groups<TL, S, G - 1, NCOMP>(v, B, tt, col, tw);
+        inv_groups<TL, S, G - 1, NBAR>(v, B, tt, col, tw, bar);
     }
 }
 
@@ -232,6 +233,15 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
             tws = (unsigned)p.NC;
             twp = p.tw_b2 + line + (long long)(tt * RL) * tws;
         }
+        // Touch this tile's boundary twiddles now, before waiting for its data: they come from L2 (a different row of
+        // the table per tile) and would otherwise be loaded right before their use (ncu: the twiddle multiplies sat
+        // on long_scoreboard for a third of all samples).
+        // (y digits; for the per-lane tables of the x digits -- 16 lines of 128 bytes per thread -- it measured as a loss)
+        if (TWB == TWB_TILE) {
+#pragma unroll
+            for (int i = 0; i < P; i += RL)
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(twp + (unsigned)((G::X3 ? sub * LP : 0) + DOP_KL(i))));
+        }
         if (V == V_H) { // touch the fy^2 entries of this tile before waiting for it
             const double* fyp = p.fy2 + o * p.row_o + m * p.row_m + tt * RL;
 #pragma unroll
@@ -330,6 +340,7 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
             //      thread forms ITS output c of the radix-3 step for its 16 positions j (three reads, one result in
             //      registers), barrier, then the sub-tile's register-blocked DFT.  Inverse: the mirror.
             const float2* __restrict__ wL = p.wL; // W_L^q, L = 3 LP
+            auto abar = [] { asm volatile("bar.sync 4, %0;" ::"n"(NCOMP) : "memory"); }; // all three groups
             float2* Bc = B + sub * LP * NB;
             if (DIR1 > 0) {
 #pragma unroll
@@ -349,8 +360,8 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                         v[i] = fx::cmul(y, __ldg(wL + sub * j));
                     }
                 }
-                cbar(); // every thread has read the three inputs of its positions
-                fwd_groups<TL, S, 0, NCOMP>(v, Bc, tt, col, tw);
+                abar(); // every thread has read the three inputs of its positions
+                fwd_groups<TL, S, 0, NB * T>(v, Bc, tt, col, tw, 1 + sub);
 #pragma unroll
                 for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], __ldg(twp + (unsigned)(sub * LP + DOP_KL(i)) * tws));
                 TL::template to_smem<GL>(v, Bc, tt, col);
@@ -358,13 +369,13 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                 TL::template from_smem<GL>(v, Bc, tt, col);
 #pragma unroll
                 for (int i = 0; i < P; ++i) v[i] = fx::cmulc(v[i], __ldg(twp + (unsigned)(sub * LP + DOP_KL(i)) * tws));
-                inv_groups<TL, S, GL, NCOMP>(v, Bc, tt, col, tw);
+                inv_groups<TL, S, GL, NB * T>(v, Bc, tt, col, tw, 1 + sub);
                 if (sub > 0) { // inputs 1, 2 of the inverse radix-3 step carry conj(W_L^{j c})
 #pragma unroll
                     for (int i = 0; i < P; ++i) v[i] = fx::cmulc(v[i], __ldg(wL + sub * (tt + i * T)));
                 }
                 TL::template to_smem<0>(v, Bc, tt, col);
-                cbar();
+                abar();
                 float2 y[P];
 #pragma unroll
                 for (int i = 0; i < P; ++i) {
@@ -381,7 +392,7 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                                         : make_float2(t2.x + t3.y, t2.y - t3.x);
                     }
                 }
-                cbar(); // all reads done before the positions are overwritten
+                abar(); // all reads done before the positions are overwritten
 #pragma unroll
                 for (int i = 0; i < P; ++i) Bc[(tt + i * T) * NB + col] = y[i];
             }
