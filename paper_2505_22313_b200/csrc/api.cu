@@ -75,6 +75,8 @@ dop_status ensure_device(dop_plan* p)
         p->pi_off[a].resize(p->ax[a].dig.size());
         for (size_t j = 0; j < p->ax[a].dig.size(); ++j) { p->pi_off[a][j] = off; off += align256(p->ax[a].dig[j].pi.size() * sizeof(int)); }
     }
+    const size_t hpair_off = off;
+    off += align256(p->hpair_items.size() * sizeof(int));
     size_t f2_off[2], g_off[2];
     for (int a = 0; a < 2; ++a) { f2_off[a] = off; off += align256(p->ax[a].f2.size() * sizeof(double)); }
     std::vector<size_t> bl_off[2];
@@ -102,6 +104,8 @@ dop_status ensure_device(dop_plan* p)
             if (!g.twb2.empty()) up(g.twb2_off, g.twb2.data(), g.twb2.size() * sizeof(float2));
     for (int a = 0; a < 2; ++a)
         for (size_t j = 0; j < p->ax[a].dig.size(); ++j) up(p->pi_off[a][j], p->ax[a].dig[j].pi.data(), p->ax[a].dig[j].pi.size() * sizeof(int));
+    up(hpair_off, p->hpair_items.data(), p->hpair_items.size() * sizeof(int));
+    p->d_hpair = p->hpair_items.empty() ? nullptr : (int*)(arena + hpair_off);
     for (int a = 0; a < 2; ++a) {
         up(f2_off[a], p->ax[a].f2.data(), p->ax[a].f2.size() * sizeof(double));
         up(g_off[a], p->ax[a].g.data(), p->ax[a].g.size() * sizeof(float));
@@ -234,6 +238,10 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
         if (d.col_type || d.cluster) d.pf_ahead = 0;
     }
     d.device = p->device;
+    if ((t.mid_op == MID_H || t.mid_op == MID_HCONJ) && d.tma > 0 && p->d_hpair != nullptr && d.n_m == 1 && d.cg0 == 0 && d.o0 == 0) {
+        d.hpair = p->d_hpair;
+        d.n_hpair = (int)(p->hpair_items.size() / 2);
+    }
     d.fx2 = p->d_f2[0];
     d.fy2 = p->d_f2[1];
     if (p->desc.band_limit) { d.fx2 = p->d_f2_bl[0][(size_t)lam]; d.fy2 = p->d_f2_bl[1][(size_t)lam]; }

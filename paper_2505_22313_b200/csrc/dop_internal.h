@@ -117,6 +117,8 @@ struct PassDesc {
     int device;           // the plan's device (function attributes are set once per device)
     long long ap_nx, ap_ny, grid_nx; // pad = 2 (generic kernel): the caller's planes are [ap_ny][ap_nx], the field window
                           // has rows of grid_nx points; plane accesses outside the aperture are masked (ap_nx = 0: no padding)
+    const int* hpair;     // (x) H pass on mirrored tile pairs (tma_hpair_kernel): n_hpair items (o_A, o_B | -1), or nullptr
+    int n_hpair;
     int tma;              // > 0: TMA column kernel (tma_col.cuh) with this many tiles in flight per CTA; nl = its bundle width
 };
 
@@ -209,6 +211,8 @@ struct dop_plan {
     size_t ws_fields = 0, ws_heff_off = 0, ws_loss_off = 0, ws_xpool_off = 0, ws_coef_off = 0, ws_gfine_off = 0, ws_bytes = 0;
     int up_lg = 0;              // log2(upsample)
     long long ap_ny = 0, ap_nx = 0; // pad = 2: the caller's aperture (desc.ny, desc.nx then hold the 2x window); 0 = no padding
+    std::vector<int> hpair_items;  // last y digit: (tile, mirror tile | -1) per work item of the paired (x) H pass; empty = unpaired
+    int* d_hpair = nullptr;
     std::vector<double*> d_f2_bl[2]; // band_limit: per-wavelength f^2 tables with the clipped bins set to 1e300
     // device tables (lazy)
     bool dev_ready = false;

@@ -540,6 +540,26 @@ dop_status build_plan(dop_plan* p)
                    p->ax[0].dig[1].fast;
     if (p->x_cluster && tu.cluster_lines > 0 && !cluster_instantiated(lx[1], tu.cluster_lines)) return DOP_ERR_INVALID_ARG;
     build_schedule(p);
+    // (x) H on mirrored tile pairs (tma_col.cuh): tile o of the last y digit holds k_low(o) + N_low k_last; its mirror
+    // holds N_low - k_low(o).  Needs a pure power-of-two last digit (slot L - 1 - i <-> k_last L - 1 - k_last).
+    p->hpair_items.clear();
+    {
+        const Axis& ay = p->ax[1];
+        const Digit& last = ay.dig.back();
+        const bool pow2 = (last.L & (last.L - 1)) == 0 && last.L >= 16;
+        if (ay.dig.size() >= 2 && pow2 && last.fast && !tu.no_mirror && p->use_tma) {
+            const long long L = last.L, nlow = ay.N / L;
+            std::vector<long long> o_of((size_t)nlow, -1);
+            for (long long o = 0; o < nlow; ++o) o_of[(size_t)(ay.kslot[(size_t)(o * L)] % nlow)] = o;
+            std::vector<int> singles;
+            for (long long o = 0; o < nlow; ++o) {
+                const long long kl = ay.kslot[(size_t)(o * L)] % nlow, om = o_of[(size_t)((nlow - kl) % nlow)];
+                if (om == o) singles.push_back((int)o);
+                else if (o < om) { p->hpair_items.push_back((int)o); p->hpair_items.push_back((int)om); }
+            }
+            for (int o : singles) { p->hpair_items.push_back(o); p->hpair_items.push_back(-1); }
+        }
+    }
     // CTAs of the MID_LOSS / plane-sum pass, in the geometry it is launched with (partials per CTA)
     p->loss_tiles = 0;
     for (const PassTmpl& t : p->fwd)

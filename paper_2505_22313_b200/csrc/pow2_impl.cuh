@@ -268,7 +268,7 @@ __device__ __forceinline__ float2 apply_h_fixed(float2 v, double c_minus_fx2, do
 // The 1/(ny nx) scale is folded into the polynomial coefficients (hk, prepared on the host: hk.s[k] =
 // scale (2 pi)^(2k+1)/(2k+1)! signed, hk.c[k] likewise for the cosine), conj H into the sign of z32.
 struct HCoef { float s[5], c[5]; };
-__device__ __forceinline__ float2 apply_h_fixed_nb(float2 v, double c_minus_fx2, double fy2, double z32, const HCoef& hk)
+__device__ __forceinline__ float2 h_fixed_nb(double c_minus_fx2, double fy2, double z32, const HCoef& hk)
 {
     const double a = c_minus_fx2 - fy2;
     const int hi = __double2hiint(a), lo = __double2loint(a);
@@ -298,7 +298,11 @@ __device__ __forceinline__ float2 apply_h_fixed_nb(float2 v, double c_minus_fx2,
     const bool prop = a >= 0.0; // evanescent bins are zeroed
     const float hx = prop ? __int_as_float(__float_as_int(co) ^ (((q + 1) & 2) << 30)) : 0.0f;
     const float hy = prop ? __int_as_float(__float_as_int(so) ^ ((q & 2) << 30)) : 0.0f;
-    return fx::cmul(v, make_float2(hx, hy));
+    return make_float2(hx, hy);
+}
+__device__ __forceinline__ float2 apply_h_fixed_nb(float2 v, double c_minus_fx2, double fy2, double z32, const HCoef& hk)
+{
+    return fx::cmul(v, h_fixed_nb(c_minus_fx2, fy2, z32, hk));
 }
 
 // Height of fine-grid point (row, x) from the caller's design layout: nearest-neighbour up-sampling of the

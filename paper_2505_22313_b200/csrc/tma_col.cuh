@@ -403,6 +403,154 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
 #undef DOP_KL
 }
 
+// ---- the (x) H sandwich on mirrored tile pairs ---------------------------------------------------------------
+// H(kx, ky) = H(kx, -ky): the tile of the last y digit that holds the frequencies k_low + N_low k_last (k_low fixed
+// by the tile, k_last by the slot) has a mirror tile holding (N_low - k_low) + N_low (L - 1 - k_last), and in the
+// digit-reversed slot order "L - 1 - k_last" is simply slot L - 1 - i: the thread that owns slots 16 tt .. 16 tt + 15
+// of tile A, acting as thread T - 1 - tt on tile B, finds in register 15 - i the point whose H it has just computed.
+// So one CTA runs the pair back to back and evaluates H (about 40 of the pass's 83 instructions per point) once
+// for both.  Work item = (column group, item q) with items[q] = (tile o_A, mirror tile o_B or -1 for the two
+// self-mirrored tiles k_low = 0, N_low / 2, which are processed alone); the tile sequence feeds the same NST-deep
+// TMA ring as tma_col_kernel.
+template <int L, int NB, int NST>
+__global__ void __launch_bounds__(TmaGeo<L, NB, V_H, NST>::THREADS, TmaGeo<L, NB, V_H, NST>::MINB)
+tma_hpair_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMaps maps, unsigned nitems)
+{
+    using G = TmaGeo<L, NB, V_H, NST>;
+    constexpr int T = G::T, NCOMP = G::NCOMP;
+    using TL = fx::Tile<L, true, NB>;
+    using S = fx::Sched<L>;
+    constexpr int GL = S::NG - 1;
+    constexpr int RL = S::radix(GL);
+    static_assert(!G::X3, "pairs of power-of-two digits only");
+    extern __shared__ __align__(128) unsigned char tm_raw[];
+    __shared__ uint64_t full[NST], done[NST];
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) {
+            tm_mbar_init(&full[s], 1);
+            tm_mbar_init(&done[s], NCOMP);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const unsigned ncg = (unsigned)p.n_cgroups;
+    const unsigned first = blockIdx.x, stride = gridDim.x;
+    const unsigned n_my = first < nitems ? (nitems - first + stride - 1) / stride : 0u;
+    const int2* __restrict__ items = reinterpret_cast<const int2*>(p.hpair);
+    auto fbuf = [&](unsigned s) -> float2* { return reinterpret_cast<float2*>(tm_raw + (size_t)s * G::STAGE_BYTES); };
+    auto item_of = [&](unsigned k, unsigned* cg) -> int2 {
+        const unsigned w = first + k * stride;
+        *cg = w % ncg;
+        return __ldg(items + w / ncg);
+    };
+
+    // ================================================================ producer warp
+    if (tid >= NCOMP) {
+        if (tid != NCOMP) return;
+        auto advance = [&](unsigned& k, int& half) {
+            unsigned cg;
+            if (half == 0 && item_of(k, &cg).y >= 0) half = 1;
+            else { half = 0; ++k; }
+        };
+        auto coords = [&](unsigned k, int half, int* c0, int* c3) {
+            unsigned cg;
+            const int2 it = item_of(k, &cg);
+            *c0 = (int)(cg + (unsigned)p.cg0) * NB;
+            *c3 = half ? it.y : it.x;
+        };
+        unsigned lk = 0, loads = 0, sk = 0, stores = 0;
+        int lhalf = 0, shalf = 0;
+        auto issue_load = [&]() {
+            const unsigned s = loads % NST;
+            int c0, c3;
+            coords(lk, lhalf, &c0, &c3);
+            tm_mbar_expect_tx(&full[s], G::FIELD_BYTES);
+#pragma unroll
+            for (int b = 0; b < G::NBOX; ++b) tm_load(fbuf(s) + b * G::LB * NB, &maps.field, &full[s], c0, 0, b * G::LB, c3);
+            ++loads;
+            advance(lk, lhalf);
+        };
+        while (loads < (unsigned)NST && lk < n_my) issue_load();
+        while (sk < n_my) {
+            const unsigned s = stores % NST;
+            tm_mbar_wait(&done[s], (stores / NST) & 1u);
+            int c0, c3;
+            coords(sk, shalf, &c0, &c3);
+#pragma unroll
+            for (int b = 0; b < G::NBOX; ++b) tm_store(&maps.field, fbuf(s) + b * G::LB * NB, c0, 0, b * G::LB, c3);
+            tm_commit();
+            ++stores;
+            advance(sk, shalf);
+            if (lk < n_my) {
+                tm_wait_read0();
+                issue_load();
+            }
+        }
+        tm_wait_all();
+        return;
+    }
+
+    // ================================================================ compute warps
+    const int col = tid % NB, tt = tid / NB;
+    const float2* __restrict__ tw = p.tw_g;
+    const double z32 = (p.mid_op == MID_HCONJ ? -p.z : p.z) * 4294967296.0; // conj H = H at the negated phase
+    HCoef hk;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { hk.s[q] = p.hk_s[q]; hk.c[q] = p.hk_c[q]; }
+#define DOP_KL(i) (((i) / RL) * (T * RL) + (i) % RL)
+    unsigned j = 0; // tiles processed so far (position in the ring)
+    for (unsigned k = 0; k < n_my; ++k) {
+        unsigned cgi;
+        const int2 it = item_of(k, &cgi);
+        const long long line0 = ((long long)cgi + p.cg0) * NB + col;
+        const long long line = line0 < p.NC ? line0 : p.NC - 1;
+        const double cfx = p.inv_lam2 - __ldg(p.fx2 + line);
+        const double* __restrict__ fyp = p.fy2 + (long long)it.x * p.row_o + tt * RL;
+#pragma unroll
+        for (int i = 0; i < P; i += RL) asm volatile("prefetch.global.L1 [%0];" ::"l"(fyp + DOP_KL(i)));
+        float2 h[P];
+        float2 v[P];
+        // ---- tile A: H evaluated
+        {
+            const unsigned s = j % NST;
+            float2* B = fbuf(s);
+            tm_mbar_wait(&full[s], (j / NST) & 1u);
+            TL::template from_smem<0>(v, B, tt, col);
+            fwd_groups<TL, S, 0, NCOMP>(v, B, tt, col, tw);
+#pragma unroll
+            for (int i = 0; i < P; ++i) {
+                h[i] = h_fixed_nb(cfx, __ldg(fyp + DOP_KL(i)), z32, hk);
+                v[i] = fx::cmul(v[i], h[i]);
+            }
+            inv_groups<TL, S, GL, NCOMP>(v, B, tt, col, tw);
+            TL::template to_smem<0>(v, B, tt, col);
+            tm_fence_async();
+            tm_mbar_arrive(&done[s]);
+            ++j;
+        }
+        // ---- tile B: the mirror tile, this thread in the place of thread T - 1 - tt, H taken from register P - 1 - i
+        if (it.y >= 0) {
+            const unsigned s = j % NST;
+            float2* B = fbuf(s);
+            const int tm = T - 1 - tt;
+            tm_mbar_wait(&full[s], (j / NST) & 1u);
+            TL::template from_smem<0>(v, B, tm, col);
+            fwd_groups<TL, S, 0, NCOMP>(v, B, tm, col, tw);
+#pragma unroll
+            for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], h[P - 1 - i]);
+            inv_groups<TL, S, GL, NCOMP>(v, B, tm, col, tw);
+            TL::template to_smem<0>(v, B, tm, col);
+            tm_fence_async();
+            tm_mbar_arrive(&done[s]);
+            ++j;
+        }
+    }
+#undef DOP_KL
+}
+
 // ---- host side -------------------------------------------------------------------------------
 typedef CUresult (*TmaEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -411,6 +559,37 @@ TmaEncodeFn tma_encode_fn();   // cuTensorMapEncodeTiled through cudaGetDriverEn
 // 4-D map of one plane for the tiles of pass p: dims (line, m, slot, o) with the pass's strides, box (nb, 1, lb, 1)
 bool tma_make_map(CUtensorMap* map, const void* base, int elem_bytes, const PassDesc& p, int nb, int lb);
 int tma_sm_count(int device);
+
+template <int L, int NB, int NST>
+static cudaError_t launch_tma_hpair(const PassDesc& p, cudaStream_t stream)
+{
+    using G = TmaGeo<L, NB, V_H, NST>;
+    static AttrOnce once;
+    static std::atomic<int> resident[64];
+    cudaError_t e = once.ensure(p.device, [&] {
+        cudaError_t a = cudaFuncSetAttribute(tma_hpair_kernel<L, NB, NST>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM);
+        if (a != cudaSuccess) return a;
+        a = cudaFuncSetAttribute(tma_hpair_kernel<L, NB, NST>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 cudaSharedmemCarveoutMaxShared);
+        if (a != cudaSuccess) return a;
+        int nb = 0;
+        a = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, tma_hpair_kernel<L, NB, NST>, G::THREADS, G::SMEM);
+        if (a != cudaSuccess) return a;
+        if (p.device >= 0 && p.device < 64) resident[p.device].store(nb < 1 ? 1 : nb);
+        return cudaSuccess;
+    });
+    if (e != cudaSuccess) return e;
+    const long long nitems = p.n_cgroups * (long long)p.n_hpair;
+    if (nitems <= 0 || nitems > 2147483647LL) return cudaErrorInvalidConfiguration;
+    TmaMaps maps;
+    memset(&maps, 0, sizeof(maps));
+    if (!tma_make_map(&maps.field, p.field, 8, p, NB, G::LB)) return cudaErrorInvalidValue;
+    const int per_sm = (p.device >= 0 && p.device < 64) ? resident[p.device].load() : 1;
+    long long grid = (long long)tma_sm_count(p.device) * (per_sm < 1 ? 1 : per_sm);
+    if (grid > nitems) grid = nitems;
+    tma_hpair_kernel<L, NB, NST><<<(unsigned)grid, G::THREADS, G::SMEM, stream>>>(p, maps, (unsigned)nitems);
+    return cudaGetLastError();
+}
 
 template <int L, int NB, int V, int TWB, int NST>
 static cudaError_t launch_tma_one(const PassDesc& p, cudaStream_t stream)
@@ -433,6 +612,9 @@ static cudaError_t launch_tma_one(const PassDesc& p, cudaStream_t stream)
     if (e != cudaSuccess) return e;
     const long long ntiles = p.n_cgroups * p.n_m * p.n_o;
     if (ntiles <= 0 || ntiles > 2147483647LL) return cudaErrorInvalidConfiguration;
+    if constexpr (V == V_H && L % 3 != 0) {
+        if (p.hpair != nullptr && p.n_m == 1) return launch_tma_hpair<L, NB, NST>(p, stream);
+    }
     TmaMaps maps;
     memset(&maps, 0, sizeof(maps));
     if (!tma_make_map(&maps.field, p.field, 8, p, NB, G::LB)) return cudaErrorInvalidValue;

@@ -177,7 +177,7 @@ def test_every_kernel_family_against_the_oracle(ny, nx, yd, xd, family):
 @pytest.mark.parametrize("tun", [
     dict(no_tma=1, col_nb=32), dict(no_tma=1, col_nb=64), dict(tma_nb=32), dict(tma_nb=16, tma_stages=3),
     dict(no_tma=1, prefetch_waves=-1), dict(no_tma=1, prefetch_waves=3), dict(force_generic=1, tile_pts=1024),
-    dict(force_generic=1, tile_pts=16384), dict(slab_mb=1, slab_streams=3),
+    dict(force_generic=1, tile_pts=16384), dict(slab_mb=1, slab_streams=3), dict(no_mirror=1), dict(no_mirror=1, tma_nb=32),
 ])
 def test_tuning_knobs_only_change_the_rounding_order(tun):
     """include/dop.h: no dop_tuning field changes a result beyond rounding order.  Every knob on a grid with two
@@ -186,6 +186,25 @@ def test_tuning_knobs_only_change_the_rounding_order(tun):
     cfg = synth.CONFIGS["C4"].scaled(4096, 16384)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
     I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(xdigits=(128, 128), ydigits=(64, 64), no_cluster=1, **tun))
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
+@pytest.mark.parametrize("ny,yd", [(6144, "384,16"), (12288, "48,256"), (8192, "16,512"), (32768, "2,128,128"), (4096, "64,64")])
+def test_H_on_mirrored_tile_pairs_against_the_oracle(ny, yd):
+    """The (x) H pass evaluates H once per pair of ky-mirrored tiles (tma_hpair_kernel): every last-digit length,
+    a 3 * 2^k first digit, a three-digit axis, against the oracle; and identical to the unpaired pass."""
+    nx = 64
+    cfg = synth.CONFIGS["C4"].scaled(ny, nx)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, tuning=dop.make_tuning(ydigits=digits(yd)))
+    assert "tma" in [l for l in plan.describe().splitlines() if "*H*" in l][0]
+    plan.close()
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(ydigits=digits(yd)))
+    I0, L0, g0 = run_l2(cfg, h, T, tuning=dop.make_tuning(ydigits=digits(yd), no_mirror=1))
+    assert np.array_equal(I, I0) and np.array_equal(g, g0) and L == L0   # same H values, same arithmetic
     Ir, Lr, gr = oracle_l2(cfg, h, T)
     check(I, Ir, "intensity")
     check(g, gr, "dL/dh")
