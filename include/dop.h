@@ -113,7 +113,8 @@ typedef struct {
                             /*       persistent TMA pipeline (tma_col.cuh)                                      */
     int32_t tma_nb;         /* 16 | 32: columns per TMA tile (0 = per-pass default)                              */
     int32_t tma_stages;     /* 1..8: tiles in flight per CTA of the TMA kernels (0 = per-pass default)          */
-    int32_t reserved[1];    /* must be 0                                                                */
+    int32_t no_stencil;     /* != 0: the Gaussian pre-filter always runs in its spectral form (ten FFT passes)  */
+                            /*       instead of the separable spatial stencil used for 2 <= sigma <= 4 px (blur.cu) */
 } dop_tuning;
 
 typedef struct {

@@ -284,6 +284,22 @@ bool zero_pruned_rows(const dop_plan* p, char* ws, int lam, cudaStream_t st)
     return cudaMemsetAsync(field + (size_t)p->ap_ny * row, 0, (size_t)(p->desc.ny - p->ap_ny) * row, st) == cudaSuccess;
 }
 
+// the Gaussian pre-filter as two stencil passes (blur.cu), one profiling slot each
+dop_status run_stencil(dop_plan* p, const float* src, float* tmp, float* dst, cudaStream_t st, const char* tag)
+{
+    long long s0 = prof_begin(p, std::string(tag) + ":blur-x", 8.0, st);
+    long long s1 = -1;
+    cudaEvent_t mid_stop = s0 >= 0 ? p->ev_stop[(size_t)s0] : nullptr, mid_start = nullptr;
+    if (p->profiling) {
+        s1 = prof_begin(p, std::string(tag) + ":blur-y", 8.0, st); // (its start event is re-recorded between the kernels)
+        if (s1 >= 0) mid_start = p->ev_start[(size_t)s1];
+    }
+    cudaError_t e = launch_blur(src, tmp, dst, p->desc.ny, p->desc.nx, p->blur_radius, p->blur_wx.data(), p->blur_wy.data(), st,
+                                mid_stop, mid_start);
+    if (s1 >= 0) prof_end(p, s1, st);
+    return e == cudaSuccess ? DOP_OK : DOP_ERR_CUDA;
+}
+
 long long gcdll(long long a, long long b) { while (b) { long long t = a % b; a = b; b = t; } return a; }
 long long lcmll(long long a, long long b) { return a / gcdll(a, b) * b; }
 
@@ -478,7 +494,12 @@ dop_status dop_propagate_fwd(dop_plan* p, const void* d_height, const float* d_t
     b.height_is_layout = true;
     b.target = d_target;
     b.intensity = d_intensity;
-    if (!p->pre.empty()) { // F0: h_eff = Re F^-1{ F{U l} G } (the layout is up-sampled inside the first read)
+    if (p->pre_stencil) { // F0 as a separable stencil: rows into the (still unused) field area, columns into h_eff
+        float* heff = (float*)(ws + p->ws_heff_off);
+        if ((s = run_stencil(p, (const float*)d_height, (float*)ws, heff, st, "pre")) != DOP_OK) return s;
+        b.height = heff;
+        b.height_is_layout = false;
+    } else if (!p->pre.empty()) { // F0: h_eff = Re F^-1{ F{U l} G } (the layout is up-sampled inside the first read)
         float* heff = (float*)(ws + p->ws_heff_off);
         Buffers pb;
         pb.real_src = d_height;
@@ -542,7 +563,7 @@ static dop_status propagate_adj(dop_plan* p, const void* d_height, const float* 
     p->state = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
-    const bool has_pre = !p->pre.empty();
+    const bool has_pre = p->desc.prefilter_sigma_px > 0.0;
     const bool pooled = p->up_lg > 0;
     const bool plain_layout = !pooled && p->desc.layout_dtype == DOP_LAYOUT_F32;
     float* xpool = (float*)(ws + p->ws_xpool_off);
@@ -570,7 +591,9 @@ static dop_status propagate_adj(dop_plan* p, const void* d_height, const float* 
         if (p->desc.loss == DOP_LOSS_NONE && !zero_pruned_rows(p, ws, lam, st)) return DOP_ERR_CUDA;
         if ((s = run(p, p->adj, lam, b, ws, st, "adj")) != DOP_OK) return s;
     }
-    if (has_pre) { // A6: the Gaussian spectrum is real and even, so the filter is self-adjoint
+    if (p->pre_stencil) { // A6 = F0 (g is even): rows into the field area (dead by now), columns back into dL/dh
+        if ((s = run_stencil(p, d_grad_height, (float*)ws, d_grad_height, st, "pre-adj")) != DOP_OK) return s;
+    } else if (has_pre) { // A6: the Gaussian spectrum is real and even, so the filter is self-adjoint
         Buffers pb;
         pb.real_src = b.grad;
         pb.real_dst = pooled ? xpool : d_grad_height;
@@ -665,7 +688,7 @@ int64_t dop_plan_launch_count(const dop_plan* p)
         }
         return n;
     };
-    int64_t n = (count(p->fwd) + count(p->adj)) * p->desc.n_lambda + 2 * count(p->pre);
+    int64_t n = (count(p->fwd) + count(p->adj)) * p->desc.n_lambda + 2 * count(p->pre) + (p->pre_stencil ? 4 : 0);
     if (p->desc.loss == DOP_LOSS_L2 || p->desc.loss == DOP_LOSS_SIMSE) n += 1; // loss / plane-sum reduction
     if (p->up_lg > 0) n += 1;                                                  // row pooling
     return n;

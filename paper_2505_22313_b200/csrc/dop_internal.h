@@ -136,6 +136,9 @@ cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n,
 // DOP_LOSS_SIMSE: plane sums -> scale s, loss, seed coefficients per wavelength (kernels_generic.cu)
 cudaError_t launch_simse_reduce(const double* scratch, long long tiles, int n_lambda, double npts, double beta,
                                 float* coef, double* d_loss, cudaStream_t stream);
+// Gaussian pre-filter as a separable spatial stencil (blur.cu): src -> tmp (rows) -> dst (columns)
+cudaError_t launch_blur(const float* src, float* tmp, float* dst, long long ny, long long nx, int radius, const float* wx,
+                        const float* wy, cudaStream_t st, cudaEvent_t mid_stop, cudaEvent_t mid_start);
 struct AdamParams { float b1, b2, c1, c2, a1, rb2, eps; }; // c1 = 1 - b1, c2 = 1 - b2 (rounded from fp64)
 // rows of the x-pooled plane -> coarse gradient [ny/r][cnx] (+ optional Adam update of the fp32 layout)
 cudaError_t launch_pool_rows(const float* xpool, float* grad, long long cny, long long cnx, int r, const AdamParams* adam,
@@ -211,6 +214,9 @@ struct dop_plan {
     size_t ws_fields = 0, ws_heff_off = 0, ws_loss_off = 0, ws_xpool_off = 0, ws_coef_off = 0, ws_gfine_off = 0, ws_bytes = 0;
     int up_lg = 0;              // log2(upsample)
     long long ap_ny = 0, ap_nx = 0; // pad = 2: the caller's aperture (desc.ny, desc.nx then hold the 2x window); 0 = no padding
+    bool pre_stencil = false;   // the pre-filter runs as a separable spatial stencil (blur.cu) instead of the spectral passes
+    int blur_radius = 0;
+    std::vector<float> blur_wx, blur_wy; // taps g[0 .. radius] of the two axes
     std::vector<int> hpair_items;  // last y digit: (tile, mirror tile | -1) per work item of the paired (x) H pass; empty = unpaired
     int* d_hpair = nullptr;
     std::vector<double*> d_f2_bl[2]; // band_limit: per-wavelength f^2 tables with the clipped bins set to 1e300

@@ -304,8 +304,8 @@ static void build_schedule(dop_plan* p)
     // adjoint
     sandwich_core(p, MID_HCONJ, !l2, &p->adj);
     p->adj.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_GRAD, "x-inv,grad", 8, 4, 4));
-    // Gaussian pre-filter (real plane -> real plane through the complex field buffer)
-    if (p->desc.prefilter_sigma_px > 0.0) {
+    // Gaussian pre-filter (real plane -> real plane through the complex field buffer), unless it runs as a stencil
+    if (p->desc.prefilter_sigma_px > 0.0 && !p->pre_stencil) {
         p->pre.push_back(mk(0, 0, +1, 0, LD_REAL, MID_NONE, ST_C64, "real,x-fwd", 4, 8));
         sandwich_core(p, MID_GAUSS, true, &p->pre);
         p->pre.push_back(mk(0, 0, -1, 0, LD_C64, MID_NONE, ST_REAL, "x-inv,real", 8, 4));
@@ -514,7 +514,6 @@ dop_status build_plan(dop_plan* p)
     // default: measured slower than whole-array launches on B200.
     if (tu.slab_mb < 0 || tu.slab_mb > 4096) return DOP_ERR_INVALID_ARG;
     p->slab_bytes = (long long)tu.slab_mb << 20;
-    if (tu.reserved[0] != 0) return DOP_ERR_INVALID_ARG;
     if (tu.tma_nb != 0 && tu.tma_nb != 16 && tu.tma_nb != 32 && tu.tma_nb != 64) return DOP_ERR_INVALID_ARG;
     if (tu.tma_stages < 0 || tu.tma_stages > 8) return DOP_ERR_INVALID_ARG;
     p->use_tma = !tu.no_tma && !p->force_generic;
@@ -539,6 +538,32 @@ dop_status build_plan(dop_plan* p)
     p->x_cluster = want_cluster && lx.size() == 2 && cluster_supported(lx[0], lx[1]) && p->ax[0].dig[0].fast &&
                    p->ax[0].dig[1].fast;
     if (p->x_cluster && tu.cluster_lines > 0 && !cluster_instantiated(lx[1], tu.cluster_lines)) return DOP_ERR_INVALID_ARG;
+    // Pre-filter as a separable spatial stencil (blur.cu) when its kernel is short: taps = the definition's own
+    // inverse DFT g[n] = (1/N) sum_k Ghat(k) cos(2 pi k n / N), n <= R = ceil(6 sigma), summed here in fp64.
+    p->pre_stencil = false;
+    if (d.prefilter_sigma_px > 0.0 && !tu.no_stencil && !p->force_generic && p->up_lg == 0 && d.layout_dtype == DOP_LAYOUT_F32) {
+        const int R = (int)std::ceil(6.0 * d.prefilter_sigma_px);
+        // (below sigma ~ 2 px the sampled spectrum is still 1e-9 or more at Nyquist: its inverse DFT then rings far beyond 6 sigma)
+        if (d.prefilter_sigma_px >= 2.05 && R <= 24 && d.nx % 8 == 0 && d.ny % 32 == 0 && d.nx >= 2 * R + 8 && d.ny >= 2 * R + 32) {
+            auto taps = [&](long long N, std::vector<float>* w) {
+                w->assign((size_t)R + 1, 0.0f);
+                const double sg = d.prefilter_sigma_px;
+                for (int n = 0; n <= R; ++n) {
+                    long double acc = 0.0L;
+                    for (long long k = 0; k < N; ++k) {
+                        const double kb = (double)(k < (N + 1) / 2 ? k : k - N), v = kb / (double)N;
+                        acc += (long double)std::exp(-2.0 * M_PI * M_PI * sg * sg * (v * v)) *
+                               cosl(2.0L * kPiL * (long double)((k * n) % N) / (long double)N);
+                    }
+                    (*w)[(size_t)n] = (float)(acc / (long double)N);
+                }
+            };
+            taps(d.nx, &p->blur_wx);
+            taps(d.ny, &p->blur_wy);
+            p->blur_radius = R;
+            p->pre_stencil = true;
+        }
+    }
     build_schedule(p);
     // (x) H on mirrored tile pairs (tma_col.cuh): tile o of the last y digit holds k_low(o) + N_low k_last; its mirror
     // holds N_low - k_low(o).  Needs a pure power-of-two last digit (slot L - 1 - i <-> k_last L - 1 - k_last).
@@ -638,10 +663,20 @@ std::string describe_plan(const dop_plan* p)
             total += t.bytes_per_point;
         }
     };
+    if (p->pre_stencil) {
+        os << "pre blur-x rows stencil radius=" << p->blur_radius << " B/pt=8 [gaussian taps along x]\n"
+           << "pre blur-y cols stencil radius=" << p->blur_radius << " B/pt=8 [gaussian taps along y]\n";
+        total += 16;
+    }
     dump("pre", p->pre);
     dump("fwd", p->fwd);
     dump("adj", p->adj);
     dump("pre-adj", p->pre);
+    if (p->pre_stencil) {
+        os << "pre-adj blur-x rows stencil radius=" << p->blur_radius << " B/pt=8 [gaussian taps along x]\n"
+           << "pre-adj blur-y cols stencil radius=" << p->blur_radius << " B/pt=8 [gaussian taps along y]\n";
+        total += 16;
+    }
     os << "algorithmic_bytes_per_point=" << total << "\n";
     if (d.n_lambda > 1)
         os << "(per wavelength; every wavelength after the first re-reads dL/dh to accumulate: +4 B/point on its last pass)\n";

@@ -36,7 +36,7 @@ class dop_tuning(C.Structure):
         ("force_generic", C.c_int32), ("col_nb", C.c_int32), ("prefetch_waves", C.c_int32), ("slab_mb", C.c_int32),
         ("slab_streams", C.c_int32), ("h_float", C.c_int32), ("tile_pts", C.c_int32), ("no_cluster", C.c_int32),
         ("no_mirror", C.c_int32), ("cluster_dsmem", C.c_int32), ("cluster_lines", C.c_int32), ("cluster_force", C.c_int32),
-        ("no_tma", C.c_int32), ("tma_nb", C.c_int32), ("tma_stages", C.c_int32), ("reserved", C.c_int32 * 1),
+        ("no_tma", C.c_int32), ("tma_nb", C.c_int32), ("tma_stages", C.c_int32), ("no_stencil", C.c_int32),
     ]
 
 
@@ -66,7 +66,7 @@ def make_tuning(xdigits: Sequence[int] = (), ydigits: Sequence[int] = (), **fiel
     for i, v in enumerate(ydigits):
         t.ydigits[i] = int(v)
     for k, v in fields.items():
-        if k not in dict(dop_tuning._fields_) or k in ("reserved", "n_xdigits", "n_ydigits"):
+        if k not in dict(dop_tuning._fields_) or k in ("n_xdigits", "n_ydigits"):
             raise TypeError(f"dop_tuning has no field {k!r}")
         setattr(t, k, int(v))
     return t

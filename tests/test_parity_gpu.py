@@ -107,12 +107,21 @@ def test_fused_l2_loss_path(ny, nx):
     assert L2 == L and np.array_equal(g2, g)
 
 
-@pytest.mark.parametrize("ny,nx", [(48, 64), (384, 512), (1024, 1536)])
-def test_prefilter_path(ny, nx):
-    cfg = synth.CONFIGS["C3"].scaled(ny, nx)
+@pytest.mark.parametrize("ny,nx,sigma,no_stencil", [(48, 64, 3.0, 0), (384, 512, 3.0, 0), (384, 512, 3.0, 1), (1024, 1536, 3.0, 0),
+                                                    (1024, 1536, 3.0, 1), (256, 640, 0.7, 0), (256, 640, 2.1, 0), (512, 512, 4.0, 0), (512, 512, 5.5, 0)])
+def test_prefilter_path(ny, nx, sigma, no_stencil):
+    """F0 / A6 against the oracle's spectral definition: as the separable spatial stencil (blur.cu; 2.05 <= sigma <= 4 px,
+    ny % 32 == 0) and in the spectral form (dop_tuning.no_stencil, ragged shapes, larger sigma)."""
+    import dataclasses
+    cfg = dataclasses.replace(synth.CONFIGS["C3"].scaled(ny, nx), sigma_px=sigma)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
     assert len(np.unique(h.cpu().numpy())) <= 256     # 256 gray levels
-    I, L, g = run_l2(cfg, h, T)
+    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, sigma, 0, DEV,
+                    tuning=dop.make_tuning(no_stencil=no_stencil))
+    stencil = "blur-x" in plan.describe()
+    plan.close()
+    assert stencil == (not no_stencil and 2.05 <= sigma <= 4.0 and ny % 32 == 0)
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(no_stencil=no_stencil))
     Ir, Lr, gr = oracle_l2(cfg, h, T)
     check(I, Ir, "intensity")
     check(g, gr, "dL/dh")
