@@ -2,7 +2,7 @@
 """bench.py -- forward+adjoint ASM throughput on B200 (BASELINE.json metric), with the kernel
 roofline and the fp64 CPU oracle timed beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C1..C5] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C1..C5] [--impl reference] [--tuning key=value ...]
 
 A step = one pass of the whole hot path (dop_propagate_fwd + dop_propagate_adj, every
 wavelength) over one batch of seeded synthetic input.  BASELINE.json's metric names no
@@ -233,6 +233,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="do not replay launch-bound configs as a CUDA graph")
+    ap.add_argument("--tuning", nargs="*", default=[], metavar="KEY=VALUE",
+                    help="dop_tuning fields for A/B measurements (include/dop.h), e.g. no_tma=1 cluster_force=1 ydigits=256,384")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     # --gpus N must be what runs: under torchrun WORLD_SIZE has to agree; a bare `bench.py --gpus N`
@@ -281,8 +283,12 @@ def main():
     warmup = max(args.warmup, 3)
     steps = max(args.steps, 1)
     flags = dop.DOP_WRITE_INTENSITY if cfg.write_intensity else 0
+    tun = {}
+    for kv in args.tuning:
+        k, v = kv.split("=")
+        tun[k] = tuple(int(x) for x in v.split(",")) if k in ("xdigits", "ydigits") else int(v)
     plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, cfg.sigma_px,
-                    flags, device=str(dev))
+                    flags, device=str(dev), tuning=dop.make_tuning(**tun) if tun else None)
     h = synth.make_height(cfg, dev)
     T = synth.make_target(cfg, dev)
     grad = torch.empty_like(h)
@@ -493,6 +499,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "c64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "points_per_step": points, "parallelism": f"replicas x{world}", "cuda_graph": bool(use_graph),
+                       "tuning": {k: (list(v) if isinstance(v, tuple) else v) for k, v in tun.items()},
                        "l2": "working set (>= 1.5 GiB) larger than the 126 MB L2; no flush between steps"
                        if points * 8 > 4 * 126e6 else "working set fits L2 (latency-bound config)",
                        "loss": loss_value},

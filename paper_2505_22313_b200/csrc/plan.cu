@@ -428,7 +428,11 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
         const bool lossp = t.mid_op == MID_LOSS && t.fft1_dir < 0 && t.fft2_dir > 0 && t.load_op == LD_C64 && t.store_op == ST_C64;
         const bool heightp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_HEIGHT && t.store_op == ST_C64 && plain_layout;
         const bool gradp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_C64 && t.store_op == ST_GRAD && plain_layout;
-        const bool has_plane = lossp || heightp || gradp;
+        // (h -> exp(i Phi) -> DFT: measured SLOWER through TMA than through the LDG/STG kernel on the bench inputs -- C4
+        // 18.6 against 13.5 ms, C5 27.9 against 20.5 -- so it goes there only when that kernel cannot run the pass:
+        // a line count that is not a multiple of 16)
+        const bool heightp_tma = heightp && d->NC % 16 != 0;
+        const bool has_plane = lossp || heightp_tma || gradp;
         // (the TMA (x) H kernel takes the phase in 32-bit fixed point: |z|/lambda < 2^19 for every wavelength)
         bool h_ok = !p->h_float;
         for (double lam : p->lambda) h_ok = h_ok && std::fabs(p->desc.z) / lam < 524288.0;
@@ -438,7 +442,7 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
             // with 32-column tiles, the register-heavy fused variants want 16 columns (two CTAs per SM)
             int nb = 32, nst = g.L <= 128 ? 3 : 2;
             if (sandwich || lossp) { nb = 16; nst = 3; }
-            if (heightp) { nb = 16; nst = g.L == 256 ? 2 : 3; }
+            if (heightp_tma) { nb = 16; nst = g.L == 256 ? 2 : 3; }
             if (g.L == 512) { nb = 16; nst = 2; }
             if (x3) { nb = 32; nst = g.L == 384 ? 2 : 3; }
             if (p->tma_nb) nb = p->tma_nb;
