@@ -2,7 +2,7 @@
 `ncu --profile-from-start off ...` (measurement aid; the timed numbers come from bench.py, never from a
 run under the profiler).
 
-  python -m paper_2505_22313_b200.ncu_step --config C5 [--labels gpurun_out/labels_C5.json] [key=value ...]
+  python -m paper_2505_22313_b200.ncu_step --config C5 [--ny NY --nx NX] [--labels gpurun_out/labels_C5.json] [key=value ...]
 
 Runs two untimed warm-up steps (the second with per-launch profiling on, to learn the pass label of
 every launch), then exactly one step inside the profiler range, and writes the labels in launch order
@@ -22,6 +22,8 @@ def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", default="C5", choices=sorted(synth.CONFIGS))
     ap.add_argument("--labels", default=None)
+    ap.add_argument("--ny", type=int, default=0, help="same recipe and optics on a smaller grid (0 = the configuration's own)")
+    ap.add_argument("--nx", type=int, default=0)
     ap.add_argument("tuning", nargs="*")
     args = ap.parse_args()
     tun = {}
@@ -29,6 +31,8 @@ def main() -> None:
         k, v = a.split("=")
         tun[k] = tuple(int(x) for x in v.split(",")) if k in ("xdigits", "ydigits") else int(v)
     cfg = synth.CONFIGS[args.config]
+    if args.ny or args.nx:
+        cfg = cfg.scaled(args.ny or cfg.ny, args.nx or cfg.nx)
     dev = "cuda:0"
     flags = dop.DOP_WRITE_INTENSITY if cfg.write_intensity else 0
     plan = dop.Plan(cfg.ny, cfg.nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, dop.DOP_LOSS_L2, cfg.sigma_px, flags, dev,
