@@ -80,7 +80,10 @@ bool tma_make_map(CUtensorMap* map, const void* base, int eb, const PassDesc& p,
     const cuuint32_t box[4] = {(cuuint32_t)nb, 1, (cuuint32_t)lb, 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUtensorMapDataType dt = eb == 8 ? CU_TENSOR_MAP_DATA_TYPE_UINT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-    const CUtensorMapL2promotion promo = nb * eb >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+    // L2 promotion no wider than one row of the box: with 64-byte rows (16 columns of an fp32 plane) a 128-byte
+    // promotion fetched every row twice (ncu at C5: the loss pass read 1.17x its algorithmic bytes)
+    const CUtensorMapL2promotion promo = nb * eb >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+                                         : nb * eb >= 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
     return enc(map, dt, 4, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }

@@ -466,7 +466,7 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
                 d->nl = nb;
                 d->n_cgroups = (d->NC + nb - 1) / nb; // (a ragged last tile is clipped by the TMA unit)
                 d->smem_bytes = (int)((long long)nst * g.L * nb * (has_plane ? 12 : 8));
-                d->threads = (int)(nb * (g.L / 16) + 32);
+                d->threads = (int)(nb * ((x3 ? g.L / 3 : g.L) / 16) + 32);
                 return;
             }
         }

@@ -16,7 +16,7 @@
 // Fused variants: plain forward / inverse (V_FWD, V_INV), the (x) H sandwich (V_H), the Gaussian
 // sandwich (V_GAUSS), and on x digits h -> exp(i Phi) -> DFT (V_HEIGHT), IDFT -> |u|^2, loss, seed ->
 // DFT (V_LOSS) and IDFT -> dL/dh (V_GRAD) with their fp32 planes staged by TMA as well.
-// Digits 3 * 2^k run one radix-3 step through the tile buffer in front of / behind three 2^k sub-tiles.
+// Digits 3 * 2^k: a thread keeps its 16 points of the three 2^k sub-tiles, radix-3 step on registers.
 #pragma once
 #include <cuda.h>
 
@@ -106,6 +106,37 @@ __device__ __forceinline__ void inv_groups(float2* v, float2* B, int tt, int col
     }
 }
 
+// Three independent sub-tiles per thread (digits 3 LP): the same walks with the three exchanges of a group boundary
+// behind ONE barrier, and three independent butterfly chains for the scheduler to interleave.
+template <class TL, class S, int G, int NBAR>
+__device__ __forceinline__ void fwd_groups3(float2 (*v)[P], float2* B, int sub_stride, int tt, int col, const float2* __restrict__ tw)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) TL::template butterflies<G, +1>(v[c], tt, tw);
+    if constexpr (G + 1 < S::NG) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) TL::template to_smem<G>(v[c], B + c * sub_stride, tt, col);
+        asm volatile("bar.sync 1, %0;" ::"n"(NBAR) : "memory");
+#pragma unroll
+        for (int c = 0; c < 3; ++c) TL::template from_smem<G + 1>(v[c], B + c * sub_stride, tt, col);
+        fwd_groups3<TL, S, G + 1, NBAR>(v, B, sub_stride, tt, col, tw);
+    }
+}
+template <class TL, class S, int G, int NBAR>
+__device__ __forceinline__ void inv_groups3(float2 (*v)[P], float2* B, int sub_stride, int tt, int col, const float2* __restrict__ tw)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) TL::template butterflies<G, -1>(v[c], tt, tw);
+    if constexpr (G > 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) TL::template to_smem<G>(v[c], B + c * sub_stride, tt, col);
+        asm volatile("bar.sync 1, %0;" ::"n"(NBAR) : "memory");
+#pragma unroll
+        for (int c = 0; c < 3; ++c) TL::template from_smem<G - 1>(v[c], B + c * sub_stride, tt, col);
+        inv_groups3<TL, S, G - 1, NBAR>(v, B, sub_stride, tt, col, tw);
+    }
+}
+
 // compile-time geometry of one instantiation
 template <int L, int NB, int V, int NST>
 struct TmaGeo {
@@ -113,7 +144,7 @@ struct TmaGeo {
     static constexpr int LP = X3 ? L / 3 : L;      // register-blocked sub-transform length
     static constexpr int NSUB = X3 ? 3 : 1;
     static constexpr int T = LP / P;               // compute threads per column
-    static constexpr int NCOMP = NB * T * NSUB;    // digits 3 LP: one thread group per sub-tile
+    static constexpr int NCOMP = NB * T;           // (digits 3 LP: a thread holds its 16 points of all three sub-tiles)
     static constexpr int THREADS = NCOMP + 32;     // + the producer warp
     static constexpr int TILE = L * NB;            // points per tile
     static constexpr int NBOX = (L + 255) / 256;   // a TMA box dimension is at most 256
@@ -206,7 +237,7 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
     }
 
     // ================================================================ compute warps
-    const int col = tid % NB, tt = (tid / NB) % T, sub = tid / (NB * T); // sub: sub-tile of a 3 LP digit (warp-uniform)
+    const int col = tid % NB, tt = tid / NB;
     const float2* __restrict__ tw = p.tw_g;
     auto cbar = [] { asm volatile("bar.sync 1, %0;" ::"n"(NCOMP) : "memory"); };
 #define DOP_KL(i) (((i) / RL) * (T * RL) + (i) % RL)
@@ -239,8 +270,9 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
         // (y digits; for the per-lane tables of the x digits -- 16 lines of 128 bytes per thread -- it measured as a loss)
         if (TWB == TWB_TILE) {
 #pragma unroll
-            for (int i = 0; i < P; i += RL)
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(twp + (unsigned)((G::X3 ? sub * LP : 0) + DOP_KL(i))));
+            for (int c = 0; c < G::NSUB; ++c)
+#pragma unroll
+                for (int i = 0; i < P; i += RL) asm volatile("prefetch.global.L1 [%0];" ::"l"(twp + (unsigned)(c * LP + DOP_KL(i))));
         }
         if (V == V_H) { // touch the fy^2 entries of this tile before waiting for it
             const double* fyp = p.fy2 + o * p.row_o + m * p.row_m + tt * RL;
@@ -336,65 +368,55 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                 TL::template to_smem<0>(v, B, tt, col);
             }
         } else {
-            // ---- digits 3 * LP: one thread group per LP-point sub-tile (c = sub, warp-uniform).  Forward: every
-            //      thread forms ITS output c of the radix-3 step for its 16 positions j (three reads, one result in
-            //      registers), barrier, then the sub-tile's register-blocked DFT.  Inverse: the mirror.
+            // ---- digits 3 * LP: a thread keeps its 16 points of all three LP-point sub-tiles (48 points; the CTA is alone
+            //      on its SM, so the registers are there), runs the radix-3 step on registers and the three sub-tile
+            //      DFTs side by side (one barrier per group boundary for the three exchanges).
             const float2* __restrict__ wL = p.wL; // W_L^q, L = 3 LP
-            auto abar = [] { asm volatile("bar.sync 4, %0;" ::"n"(NCOMP) : "memory"); }; // all three groups
-            float2* Bc = B + sub * LP * NB;
+            float2 w3[3][P];
             if (DIR1 > 0) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) TL::template from_smem<0>(w3[c], B + c * LP * NB, tt, col);
+#pragma unroll
+                for (int i = 0; i < P; ++i) { // radix-3 step (block length L, stride LP), outputs c = 1, 2 times W_L^{j c}
+                    const int j = tt + i * T;
+                    const float2 a = w3[0][i], b = w3[1][i], c = w3[2][i];
+                    const float2 t1 = fx::cadd(b, c), d = fx::csub(b, c);
+                    const float2 t2 = make_float2(a.x - 0.5f * t1.x, a.y - 0.5f * t1.y);
+                    const float2 t3 = make_float2(HS3 * d.x, HS3 * d.y);
+                    w3[0][i] = fx::cadd(a, t1);
+                    w3[1][i] = fx::cmul(make_float2(t2.x + t3.y, t2.y - t3.x), __ldg(wL + j));     // t2 - i t3
+                    w3[2][i] = fx::cmul(make_float2(t2.x - t3.y, t2.y + t3.x), __ldg(wL + 2 * j)); // t2 + i t3
+                }
+                fwd_groups3<TL, S, 0, NCOMP>(w3, B, LP * NB, tt, col, tw);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                    for (int i = 0; i < P; ++i) w3[c][i] = fx::cmul(w3[c][i], __ldg(twp + (unsigned)(c * LP + DOP_KL(i)) * tws));
+                    TL::template to_smem<GL>(w3[c], B + c * LP * NB, tt, col);
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    TL::template from_smem<GL>(w3[c], B + c * LP * NB, tt, col);
+#pragma unroll
+                    for (int i = 0; i < P; ++i) w3[c][i] = fx::cmulc(w3[c][i], __ldg(twp + (unsigned)(c * LP + DOP_KL(i)) * tws));
+                }
+                inv_groups3<TL, S, GL, NCOMP>(w3, B, LP * NB, tt, col, tw);
 #pragma unroll
                 for (int i = 0; i < P; ++i) {
                     const int j = tt + i * T;
-                    const float2* e = B + j * NB + col;
-                    const float2 a = e[0], b = e[LP * NB], c = e[2 * LP * NB];
-                    const float2 t1 = fx::cadd(b, c);
-                    if (sub == 0) {
-                        v[i] = fx::cadd(a, t1);
-                    } else {
-                        const float2 d = fx::csub(b, c);
-                        const float2 t2 = make_float2(a.x - 0.5f * t1.x, a.y - 0.5f * t1.y);
-                        const float2 t3 = make_float2(HS3 * d.x, HS3 * d.y);
-                        const float2 y = sub == 1 ? make_float2(t2.x + t3.y, t2.y - t3.x)  // t2 - i t3
-                                                  : make_float2(t2.x - t3.y, t2.y + t3.x); // t2 + i t3
-                        v[i] = fx::cmul(y, __ldg(wL + sub * j));
-                    }
+                    const float2 a = w3[0][i];
+                    const float2 b = fx::cmulc(w3[1][i], __ldg(wL + j));
+                    const float2 c = fx::cmulc(w3[2][i], __ldg(wL + 2 * j));
+                    const float2 t1 = fx::cadd(b, c), d = fx::csub(b, c);
+                    const float2 t2 = make_float2(a.x - 0.5f * t1.x, a.y - 0.5f * t1.y);
+                    const float2 t3 = make_float2(HS3 * d.x, HS3 * d.y);
+                    w3[0][i] = fx::cadd(a, t1);
+                    w3[1][i] = make_float2(t2.x - t3.y, t2.y + t3.x); // inverse: t2 + i t3
+                    w3[2][i] = make_float2(t2.x + t3.y, t2.y - t3.x);
                 }
-                abar(); // every thread has read the three inputs of its positions
-                fwd_groups<TL, S, 0, NB * T>(v, Bc, tt, col, tw, 1 + sub);
 #pragma unroll
-                for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], __ldg(twp + (unsigned)(sub * LP + DOP_KL(i)) * tws));
-                TL::template to_smem<GL>(v, Bc, tt, col);
-            } else {
-                TL::template from_smem<GL>(v, Bc, tt, col);
-#pragma unroll
-                for (int i = 0; i < P; ++i) v[i] = fx::cmulc(v[i], __ldg(twp + (unsigned)(sub * LP + DOP_KL(i)) * tws));
-                inv_groups<TL, S, GL, NB * T>(v, Bc, tt, col, tw, 1 + sub);
-                if (sub > 0) { // inputs 1, 2 of the inverse radix-3 step carry conj(W_L^{j c})
-#pragma unroll
-                    for (int i = 0; i < P; ++i) v[i] = fx::cmulc(v[i], __ldg(wL + sub * (tt + i * T)));
-                }
-                TL::template to_smem<0>(v, Bc, tt, col);
-                abar();
-                float2 y[P];
-#pragma unroll
-                for (int i = 0; i < P; ++i) {
-                    const float2* e = B + (tt + i * T) * NB + col;
-                    const float2 a = e[0], b = e[LP * NB], c = e[2 * LP * NB];
-                    const float2 t1 = fx::cadd(b, c);
-                    if (sub == 0) {
-                        y[i] = fx::cadd(a, t1);
-                    } else {
-                        const float2 d = fx::csub(b, c);
-                        const float2 t2 = make_float2(a.x - 0.5f * t1.x, a.y - 0.5f * t1.y);
-                        const float2 t3 = make_float2(HS3 * d.x, HS3 * d.y);
-                        y[i] = sub == 1 ? make_float2(t2.x - t3.y, t2.y + t3.x)  // inverse: t2 + i t3
-                                        : make_float2(t2.x + t3.y, t2.y - t3.x);
-                    }
-                }
-                abar(); // all reads done before the positions are overwritten
-#pragma unroll
-                for (int i = 0; i < P; ++i) Bc[(tt + i * T) * NB + col] = y[i];
+                for (int c = 0; c < 3; ++c) TL::template to_smem<0>(w3[c], B + c * LP * NB, tt, col);
             }
         }
         tm_fence_async();          // this thread's writes to the tile are visible to the TMA store

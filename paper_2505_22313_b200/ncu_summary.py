@@ -22,7 +22,7 @@ METRICS = [
     ("time_us", "gpu__time_duration.sum"),
     ("dram_bytes_read", "dram__bytes_read.sum"),
     ("dram_bytes_write", "dram__bytes_write.sum"),
-    ("dram_pct", "dram__throughput.avg.pct_of_peak_sustained_elapsed"),
+    ("dram_pct", "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed"),
     ("issue_active_pct", "smsp__issue_active.avg.pct_of_peak_sustained_active"),
     ("warps_active_pct", "sm__warps_active.avg.pct_of_peak_sustained_active"),
     ("l1_wavefronts_pct", "l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed"),
