@@ -280,6 +280,13 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
             for (int i = 0; i < P; i += RL) asm volatile("prefetch.global.L1 [%0];" ::"l"(fyp + DOP_KL(i)));
         }
 
+        // Per-lane boundary twiddles (x digits: 16 table lines per thread, from L2) are fetched into registers BEFORE
+        // the wait for the tile, so their latency hides behind it; the loss pass uses them twice.
+        float2 twv[TWB == TWB_LANE && !G::X3 ? P : 1];
+        if (TWB == TWB_LANE && !G::X3) {
+#pragma unroll
+            for (int i = 0; i < P; ++i) twv[i] = __ldg(twp + (unsigned)DOP_KL(i) * tws);
+        }
         tm_mbar_wait(&full[s], (k / NST) & 1u);
 
         float2 v[P];
@@ -298,7 +305,10 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                 fwd_groups<TL, S, 0, NCOMP>(v, B, tt, col, tw);
             } else {
                 TL::template from_smem<GL>(v, B, tt, col);
-                if (TWB != TWB_NONE) {
+                if (TWB == TWB_LANE) {
+#pragma unroll
+                    for (int i = 0; i < P; ++i) v[i] = fx::cmulc(v[i], twv[i]);
+                } else if (TWB != TWB_NONE) {
 #pragma unroll
                     for (int i = 0; i < P; ++i) v[i] = fx::cmulc(v[i], __ldg(twp + (unsigned)DOP_KL(i) * tws));
                 }
@@ -351,7 +361,10 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
             else if (DIR2 < 0) inv_groups<TL, S, GL, NCOMP>(v, B, tt, col, tw);
             // ---- store (+ boundary twiddle after a forward DFT, + epilogue)
             if (LAST > 0) {
-                if (TWB != TWB_NONE) {
+                if (TWB == TWB_LANE) {
+#pragma unroll
+                    for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], twv[i]);
+                } else if (TWB != TWB_NONE) {
 #pragma unroll
                     for (int i = 0; i < P; ++i) v[i] = fx::cmul(v[i], __ldg(twp + (unsigned)DOP_KL(i) * tws));
                 }
