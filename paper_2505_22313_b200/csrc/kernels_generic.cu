@@ -24,6 +24,17 @@ __device__ __forceinline__ float2 cmulc(float2 a, float2 b) // a * conj(b)
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 
+// a / d for the small non-negative index arithmetic of this file (a < 2^20, d < 2^14): one multiply by the
+// precomputed reciprocal instead of a ~25-instruction integer division.  (a + 1/2) inv is off by less than
+// a 2^-22 / d < 1/(2 d), and the fractional part of (a + 1/2)/d is at least 1/(2 d), so the floor is exact.
+struct FastDiv {
+    int d;
+    float inv;
+    __device__ __forceinline__ explicit FastDiv(int dd) : d(dd), inv(1.0f / (float)dd) {}
+    __device__ __forceinline__ int div(int a) const { return __float2int_rz(((float)a + 0.5f) * inv); }
+    __device__ __forceinline__ void divmod(int a, int* q, int* r) const { *q = div(a); *r = a - *q * d; }
+};
+
 // one radix-r butterfly, DIR = +1: exp(-2 pi i pc/r), DIR = -1: exp(+...)
 template <int DIR>
 __device__ __forceinline__ void bfly2(float2* v)
@@ -117,11 +128,15 @@ __device__ void prime_step(float2* s, float2* s2, const PassDesc& p, int nl_eff,
     const float2* __restrict__ wL = p.wL;
     const int m = nq / r, tws = L / nq, twr = L / r, per_line = L / r, h = (r - 1) / 2;
     const int total = nl_eff * L;
+    const FastDiv d_nl(nl_eff), d_L(L), d_nq(nq), d_m(m), d_pl(per_line);
     if (DIR < 0 && m > 1) {
         for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
             int l, i;
-            if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
-            const int pos = i % nq, c = pos / m, j = pos - c * m;
+            if (COL) d_nl.divmod(idx, &i, &l);
+            else d_L.divmod(idx, &l, &i);
+            int blk, pos, c, j;
+            d_nq.divmod(i, &blk, &pos);
+            d_m.divmod(pos, &c, &j);
             if (c > 0 && j > 0) s[l * sl + i * se] = cmulc(s[l * sl + i * se], __ldg(wL + j * c * tws));
         }
         __syncthreads();
@@ -129,9 +144,10 @@ __device__ void prime_step(float2* s, float2* s2, const PassDesc& p, int nl_eff,
     const int items = nl_eff * per_line * (h + 1);
     for (int it = threadIdx.x; it < items; it += blockDim.x) {
         int l, jj, kk;
-        if (COL) { l = it % nl_eff; const int rest = it / nl_eff; jj = rest % per_line; kk = rest / per_line; }
-        else { jj = it % per_line; const int rest = it / per_line; l = rest % nl_eff; kk = rest / nl_eff; }
-        const int b = jj / m, j = jj - b * m;
+        int rest, b, j;
+        if (COL) { d_nl.divmod(it, &rest, &l); d_pl.divmod(rest, &kk, &jj); }
+        else { d_pl.divmod(it, &rest, &jj); d_nl.divmod(rest, &kk, &l); }
+        d_m.divmod(jj, &b, &j);
         const int base = l * sl + (b * nq + j) * se, step = m * se;
         const float2 x0 = s[base];
         if (kk == 0) {
@@ -190,10 +206,12 @@ __device__ void tile_fft(float2* s, float2* s2, const PassDesc& p, int nl_eff, i
         const int tws = L / nq;     // W_{n_q}^x = wL[x * tws]
         const int per_line = L / r;
         const int nbf = nl_eff * per_line;
+        const FastDiv d_nl(nl_eff), d_pl(per_line), d_m(m);
         for (int bf = threadIdx.x; bf < nbf; bf += blockDim.x) {
-            int l, jj;
-            if (COL) { l = bf % nl_eff; jj = bf / nl_eff; } else { jj = bf % per_line; l = bf / per_line; }
-            const int b = jj / m, j = jj - b * m;
+            int l, jj, b, j;
+            if (COL) d_nl.divmod(bf, &jj, &l);
+            else d_pl.divmod(bf, &l, &jj);
+            d_m.divmod(jj, &b, &j);
             float2* e = s + l * sl + (b * nq + j) * se;
             const int step = m * se;
             float2 v[7];
@@ -247,7 +265,7 @@ __device__ __forceinline__ long long plane_offset(const PassDesc& p, long long o
 }
 
 template <bool COL>
-__global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
+__global__ void __launch_bounds__(256, 4) tile_pass_kernel(const PassDesc p)
 {
     extern __shared__ float2 s[];
     __shared__ double red[8];
@@ -268,6 +286,7 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
     const int se = COL ? nl_eff : 1;
     const long long ls = p.SCc, es = p.es;
     const int total = nl_eff * L;
+    const FastDiv d_nl(nl_eff), d_L(L);
     float2* s2 = s + p.nl * L; // scratch of the prime-radix steps (the plan doubles smem_bytes for such digits)
     const long long r0 = p.r_from ? m : c0; // boundary-twiddle r of line 0 (x digit: r = c)
     const int r_per_line = p.r_from ? 0 : 1;
@@ -275,7 +294,8 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
     // ---- load (+ prologue op, + conj boundary twiddle before an inverse DFT)
     for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
         int l, i;
-        if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+        if (COL) d_nl.divmod(idx, &i, &l);
+        else d_L.divmod(idx, &l, &i);
         const long long off = base + l * ls + i * es;
         float2 v;
         const long long poff = (p.load_op == LD_HEIGHT || p.load_op == LD_SEED) ? plane_offset(p, off) : off;
@@ -313,7 +333,8 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
         const long long row0 = o * p.row_o + m * p.row_m;
         for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
             int l, i;
-            if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+            if (COL) d_nl.divmod(idx, &i, &l);
+        else d_L.divmod(idx, &l, &i);
             const long long row = row0 + i * p.row_i;
             const long long col = c0 + l;
             float2 v = s[l * sl + i * se];
@@ -341,7 +362,8 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
         double acc = 0.0;
         for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
             int l, i;
-            if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+            if (COL) d_nl.divmod(idx, &i, &l);
+        else d_L.divmod(idx, &l, &i);
             const long long off = base + l * ls + i * es;
             float2 v = s[l * sl + i * se];
             const long long poff = plane_offset(p, off);
@@ -378,7 +400,8 @@ __global__ void __launch_bounds__(256) tile_pass_kernel(const PassDesc p)
     // ---- store (+ boundary twiddle after a forward DFT, + epilogue op)
     for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
         int l, i;
-        if (COL) { l = idx % nl_eff; i = idx / nl_eff; } else { i = idx % L; l = idx / L; }
+        if (COL) d_nl.divmod(idx, &i, &l);
+        else d_L.divmod(idx, &l, &i);
         const long long off = base + l * ls + i * es;
         float2 v = s[l * sl + i * se];
         if (p.tw_b != nullptr && last_dir > 0) {

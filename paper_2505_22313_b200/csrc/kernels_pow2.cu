@@ -175,7 +175,6 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
     const bool col = p.col_type != 0;
     if (p.tw_g == nullptr || !pow2_supported(p.L, col)) return cudaSuccess;
     if (col ? !(p.nl == 16 || p.nl == 32 || p.nl == 64) : p.nl != pow2_lines(p.L, false)) return cudaSuccess;
-    if (p.NC % p.nl != 0) return cudaSuccess;
     const int v = pass_variant(p);
     if (v < 0) return cudaSuccess;
     if ((v == V_H || v == V_GAUSS) && (!col || p.row_i != 1)) return cudaSuccess;
@@ -192,6 +191,7 @@ cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* 
             return e;
         }
     }
+    if (p.NC % p.nl != 0) return cudaSuccess; // (a ragged last tile: only the TMA kernels clip it; else the generic kernel)
     if (p.L % 3 == 0) {
         switch (p.L / 3) {
         case 16: e = launch_x3<16>(p, v, twb, stream); break;
