@@ -218,6 +218,10 @@ PassDesc resolve(const dop_plan* p, const PassTmpl& t, int lam, const Buffers& b
     d.scale = (float)(1.0 / (double)npts);
     d.seed_coef = (float)(4.0 / (double)nap);
     if (p->ap_nx > 0 && t.axis == 0) { d.ap_nx = p->ap_nx; d.ap_ny = p->ap_ny; d.grid_nx = p->desc.nx; }
+    // pad = 2: a pass that touches the caller's planes masks them to the aperture -- in the TMA kernels (tile maps of
+    // the aperture's shape) or in the generic kernel; it must never reach the LDG/STG kernels, which do not
+    if (d.ap_nx > 0 && d.tma == 0 && (t.load_op != LD_C64 || t.store_op != ST_C64 || t.mid_op == MID_LOSS)) d.tw_g = nullptr;
+    if (d.ap_nx > 0 && d.tma > 0 && (d.n_m != 1 || p->ap_nx % 4 != 0)) { d.tma = 0; d.tw_g = nullptr; pass_geometry(p, t, &d, false); d.tw_g = nullptr; }
     d.inv_lam2 = 1.0 / (lambda * lambda);
     d.z = p->desc.z;
     d.h_fixed = (std::fabs(p->desc.z) / lambda < 524288.0 && !p->h_float) ? 1 : 0;

@@ -65,12 +65,13 @@ int tma_sm_count(int device)
     return n;
 }
 
-bool tma_make_map(CUtensorMap* map, const void* base, int eb, const PassDesc& p, int nb, int lb)
+bool tma_make_map(CUtensorMap* map, const void* base, int eb, const PassDesc& p, int nb, int lb, long long slots, long long so)
 {
     TmaEncodeFn enc = tma_encode_fn();
     if (enc == nullptr || base == nullptr || ((uintptr_t)base & 15) != 0) return false;
-    const cuuint64_t dims[4] = {(cuuint64_t)p.NC, (cuuint64_t)p.n_m, (cuuint64_t)p.L, (cuuint64_t)(p.n_o + p.o0)};
-    cuuint64_t strides[3] = {(cuuint64_t)p.SM * eb, (cuuint64_t)p.es * eb, (cuuint64_t)p.SO * eb};
+    // (slots / so: pad = 2 planes -- only the first L/2 slots of a line lie inside the aperture, whose rows are ap_nx long)
+    const cuuint64_t dims[4] = {(cuuint64_t)p.NC, (cuuint64_t)p.n_m, (cuuint64_t)(slots > 0 ? slots : p.L), (cuuint64_t)(p.n_o + p.o0)};
+    cuuint64_t strides[3] = {(cuuint64_t)p.SM * eb, (cuuint64_t)p.es * eb, (cuuint64_t)(so > 0 ? so : p.SO) * eb};
     for (int i = 0; i < 3; ++i) {
         if (dims[i + 1] == 1 && strides[i] == 0) strides[i] = 16; // (a dimension of extent 1: the stride is never used)
         if (strides[i] % 16 != 0 || strides[i] >= (1ull << 40)) return false;

@@ -214,7 +214,10 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
                  (col_type ? (lines % 16 == 0 || !tu_no_tma) : lines % pow2_lines(d.L, false) == 0);
         // pad = 2: the fused x passes mask their plane accesses to the aperture, which only the generic kernel
         // implements (the plain x passes and every y pass keep the specialised kernels)
-        if (p->ap_nx > 0 && a == 0 && j == 0) d.fast = false;
+        // ... unless the x axis has two digits and the first is a power of two: its fused passes then run on the TMA
+        // kernels, where the TMA unit itself masks the planes to the aperture (resolve() sends anything else to the generic kernel)
+        const bool pad_tma = Ls.size() == 2 && (d.L & (d.L - 1)) == 0 && d.L >= 16 && !tu_no_tma && !p->force_generic;
+        if (p->ap_nx > 0 && a == 0 && j == 0 && !pad_tma) d.fast = false;
         if (d.fast) d.twg = pow2_group_twiddles(d.L);
         if (d.fast && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
             const long long Nj = d.L * d.st;
@@ -431,7 +434,7 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
         // (h -> exp(i Phi) -> DFT: measured SLOWER through TMA than through the LDG/STG kernel on the bench inputs -- C4
         // 18.6 against 13.5 ms, C5 27.9 against 20.5 -- so it goes there only when that kernel cannot run the pass:
         // a line count that is not a multiple of 16)
-        const bool heightp_tma = heightp && d->NC % 16 != 0;
+        const bool heightp_tma = heightp && (d->NC % 16 != 0 || p->ap_nx > 0); // (pad = 2: only the TMA kernel masks)
         const bool has_plane = lossp || heightp_tma || gradp;
         // (the TMA (x) H kernel takes the phase in 32-bit fixed point: |z|/lambda < 2^19 for every wavelength)
         bool h_ok = !p->h_float;
@@ -680,6 +683,11 @@ std::string describe_plan(const dop_plan* p)
         os << "pre-adj blur-x rows stencil radius=" << p->blur_radius << " B/pt=8 [gaussian taps along x]\n"
            << "pre-adj blur-y cols stencil radius=" << p->blur_radius << " B/pt=8 [gaussian taps along y]\n";
         total += 16;
+    }
+    if (!p->hpair_items.empty()) {
+        size_t yp = 0;
+        for (size_t i = 1; i < p->hpair_items.size(); i += 2) yp += p->hpair_items[i] >= 0;
+        os << "H on mirrored tiles: " << p->hpair_items.size() / 2 << " work items per column group (" << yp << " ky-mirror pairs)\n";
     }
     os << "algorithmic_bytes_per_point=" << total << "\n";
     if (d.n_lambda > 1)

@@ -298,6 +298,8 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                     for (int i = 0; i < P; ++i) {
                         const float ph = Pl[(tt + i * T) * NB + col] * p.phase_coef; // Eq. (1) in turns
                         sincos_turns(ph, &v[i].y, &v[i].x);                          // Eq. (2), E_in = 1
+                        // pad = 2: slots tt + i T >= L/2, i.e. registers i >= 8, lie outside the aperture: zero amplitude
+                        if (i >= P / 2 && p.ap_nx > 0) v[i] = make_float2(0.0f, 0.0f);
                     }
                 } else {
                     TL::template from_smem<0>(v, B, tt, col);
@@ -340,7 +342,8 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                 for (int i = 0; i < P; ++i) {
                     float* tp = Pl + (tt + i * T) * NB + col;
                     const float I = v[i].x * v[i].x + v[i].y * v[i].y; // F6
-                    const float d = I - *tp;                           // F7
+                    float d = I - *tp;                                 // F7
+                    if (i >= P / 2 && p.ap_nx > 0) d = 0.0f;           // pad = 2: outside the aperture, no loss term, zero seed
                     acc += (double)d * (double)d;
                     const float g = p.seed_coef * d;                   // A1: 2 gI = 4 (I - T)/N
                     v[i] = make_float2(g * v[i].x, g * v[i].y);
@@ -592,7 +595,8 @@ typedef CUresult (*TmaEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, v
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 TmaEncodeFn tma_encode_fn();   // cuTensorMapEncodeTiled through cudaGetDriverEntryPoint (no link against libcuda)
 // 4-D map of one plane for the tiles of pass p: dims (line, m, slot, o) with the pass's strides, box (nb, 1, lb, 1)
-bool tma_make_map(CUtensorMap* map, const void* base, int elem_bytes, const PassDesc& p, int nb, int lb);
+bool tma_make_map(CUtensorMap* map, const void* base, int elem_bytes, const PassDesc& p, int nb, int lb, long long slots = 0,
+                  long long so = 0);
 int tma_sm_count(int device);
 
 template <int L, int NB, int NST>
@@ -653,12 +657,16 @@ static cudaError_t launch_tma_one(const PassDesc& p, cudaStream_t stream)
     TmaMaps maps;
     memset(&maps, 0, sizeof(maps));
     if (!tma_make_map(&maps.field, p.field, 8, p, NB, G::LB)) return cudaErrorInvalidValue;
+    // pad = 2: the planes are [ap_ny][ap_nx]; along a line only slots < L/2 (x < ap_nx) exist, the TMA unit fills
+    // the rest of a loaded tile with zeros and clips the stored one (needs the line to be the whole x axis: n_m = 1)
+    const long long pslots = p.ap_nx > 0 ? p.L / 2 : 0, pso = p.ap_nx > 0 ? p.ap_nx : 0;
+    if (p.ap_nx > 0 && (p.n_m != 1 || G::PIN == false)) return cudaErrorInvalidValue;
     if (G::PIN) {
         const float* src = V == V_LOSS ? p.plane_in : p.height;
-        if (!tma_make_map(&maps.pin, src, 4, p, NB, G::LB)) return cudaErrorInvalidValue;
+        if (!tma_make_map(&maps.pin, src, 4, p, NB, G::LB, pslots, pso)) return cudaErrorInvalidValue;
     }
     if (V == V_GRAD || (V == V_LOSS && p.write_intensity)) {
-        if (!tma_make_map(&maps.pout, p.plane_out, 4, p, NB, G::LB)) return cudaErrorInvalidValue;
+        if (!tma_make_map(&maps.pout, p.plane_out, 4, p, NB, G::LB, pslots, pso)) return cudaErrorInvalidValue;
     }
     const int per_sm = (p.device >= 0 && p.device < 64) ? resident[p.device].load() : 1;
     long long grid = (long long)tma_sm_count(p.device) * (per_sm < 1 ? 1 : per_sm);

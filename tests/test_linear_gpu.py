@@ -19,13 +19,17 @@ def check(a, b, what):
 
 
 @pytest.mark.parametrize("ny,nx,z,bl", [(6, 10, 20e-6, 0), (48, 64, 0.2e-3, 1), (96, 200, 1e-3, 1), (512, 384, 2e-3, 0),
-                                        (512, 384, 2e-3, 1), (300, 1000, 5e-3, 1), (2048, 4096, 20e-3, 1)])
+                                        (512, 384, 2e-3, 1), (300, 1000, 5e-3, 1), (2048, 4096, 20e-3, 1),
+                                        (256, 8192, 5e-3, 1), (96, 16384, 5e-3, 0)])   # two x digits: aperture masked by the TMA unit
 def test_padded_l2_path_against_the_linear_oracle(ny, nx, z, bl):
     cfg = synth.CONFIGS["C4"].scaled(ny, nx)
     lambdas, n_refr = (550e-9, 633e-9), (1.5, 1.47)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
     plan = dop.Plan(ny, nx, cfg.pitch, lambdas, n_refr, z, dop.DOP_LOSS_L2, 0.0, dop.DOP_WRITE_INTENSITY, DEV, pad=2, band_limit=bl)
-    assert "pad=2" in plan.describe()
+    text = plan.describe()
+    assert "pad=2" in text
+    if nx >= 8192:   # the window's x axis has two digits: the fused x passes run on the TMA kernels, not on the generic one
+        assert "col tma" in [l for l in text.splitlines() if "loss,seed" in l][0], text
     inten = torch.full((2, ny, nx), float("nan"), dtype=torch.float32, device=DEV)
     grad = torch.full_like(h, float("nan"))
     loss = torch.zeros(1, dtype=torch.float64, device=DEV)

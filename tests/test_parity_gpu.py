@@ -201,18 +201,22 @@ def test_tuning_knobs_only_change_the_rounding_order(tun):
     assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
 
 
-@pytest.mark.parametrize("ny,yd", [(6144, "384,16"), (12288, "48,256"), (8192, "16,512"), (32768, "2,128,128"), (4096, "64,64")])
-def test_H_on_mirrored_tile_pairs_against_the_oracle(ny, yd):
-    """The (x) H pass evaluates H once per pair of ky-mirrored tiles (tma_hpair_kernel): every last-digit length,
-    a 3 * 2^k first digit, a three-digit axis, against the oracle; and identical to the unpaired pass."""
-    nx = 64
+@pytest.mark.parametrize("ny,yd,nx,xd", [(6144, "384,16", 64, "64"), (12288, "48,256", 64, "64"), (8192, "16,512", 128, "128"),
+                                         (32768, "2,128,128", 64, "64"), (4096, "64,64", 4096, "64,64"),
+                                         (2048, "16,128", 8192, "32,256"), (512, "8,64", 16384, "2,64,128")])
+def test_H_on_mirrored_tile_pairs_against_the_oracle(ny, yd, nx, xd):
+    """The (x) H pass evaluates H once per group of up to four kx- / ky-mirrored tiles (tma_hpair_kernel): every
+    last-digit length, a 3 * 2^k first digit, one-, two- and three-digit axes, against the oracle; and bitwise
+    identical to the unpaired pass (same H values, same arithmetic)."""
     cfg = synth.CONFIGS["C4"].scaled(ny, nx)
     h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
-    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, tuning=dop.make_tuning(ydigits=digits(yd)))
-    assert "tma" in [l for l in plan.describe().splitlines() if "*H*" in l][0]
+    tun = dict(ydigits=digits(yd), xdigits=digits(xd), no_cluster=1)
+    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, tuning=dop.make_tuning(**tun))
+    text = plan.describe()
     plan.close()
-    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(ydigits=digits(yd)))
-    I0, L0, g0 = run_l2(cfg, h, T, tuning=dop.make_tuning(ydigits=digits(yd), no_mirror=1))
+    assert "tma" in [l for l in text.splitlines() if "*H*" in l][0] and "H on mirrored tiles" in text, text
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(**tun))
+    I0, L0, g0 = run_l2(cfg, h, T, tuning=dop.make_tuning(no_mirror=1, **tun))
     assert np.array_equal(I, I0) and np.array_equal(g, g0) and L == L0   # same H values, same arithmetic
     Ir, Lr, gr = oracle_l2(cfg, h, T)
     check(I, Ir, "intensity")
