@@ -435,7 +435,12 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
         // 18.6 against 13.5 ms, C5 27.9 against 20.5 -- so it goes there only when that kernel cannot run the pass:
         // a line count that is not a multiple of 16)
         const bool heightp_tma = heightp && (d->NC % 16 != 0 || p->ap_nx > 0); // (pad = 2: only the TMA kernel masks)
-        const bool has_plane = lossp || heightp_tma || gradp;
+        // the split loss flavours: IDFT -> u, |u|^2 [, plane sums]  and  seed from u and dL/dI (or T) -> DFT
+        const bool statp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_C64 &&
+                           (t.store_op == ST_C64_INTENSITY || t.store_op == ST_C64_STATS) && t.axis == 0;
+        const bool seedp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.store_op == ST_C64 &&
+                           (t.load_op == LD_SEED || t.load_op == LD_SEED_SIMSE) && t.axis == 0;
+        const bool has_plane = lossp || heightp_tma || gradp || statp || seedp;
         // (the TMA (x) H kernel takes the phase in 32-bit fixed point: |z|/lambda < 2^19 for every wavelength)
         bool h_ok = !p->h_float;
         for (double lam : p->lambda) h_ok = h_ok && std::fabs(p->desc.z) / lam < 524288.0;
@@ -444,7 +449,7 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
             // measured per variant at L = 256 (C4): plain passes and the dL/dh store are near the pattern's ceiling
             // with 32-column tiles, the register-heavy fused variants want 16 columns (two CTAs per SM)
             int nb = 32, nst = g.L <= 128 ? 3 : 2;
-            if (sandwich || lossp) { nb = 16; nst = 3; }
+            if (sandwich || lossp || statp || seedp) { nb = 16; nst = 3; }
             if (heightp_tma) { nb = 16; nst = g.L == 256 ? 2 : 3; }
             if (g.L == 512) { nb = 16; nst = 2; }
             if (x3) { nb = 32; nst = g.L == 384 ? 2 : 3; }

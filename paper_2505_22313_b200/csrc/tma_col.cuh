@@ -15,7 +15,8 @@
 //
 // Fused variants: plain forward / inverse (V_FWD, V_INV), the (x) H sandwich (V_H), the Gaussian
 // sandwich (V_GAUSS), and on x digits h -> exp(i Phi) -> DFT (V_HEIGHT), IDFT -> |u|^2, loss, seed ->
-// DFT (V_LOSS) and IDFT -> dL/dh (V_GRAD) with their fp32 planes staged by TMA as well.
+// DFT (V_LOSS), IDFT -> dL/dh (V_GRAD), and the split loss flavours of DOP_LOSS_NONE / DOP_LOSS_SIMSE (IDFT -> u, |u|^2
+// [, plane sums]: V_STOTHER; seed from u and a plane -> DFT: V_LDOTHER) with their fp32 planes staged by TMA as well.
 // Digits 3 * 2^k: a thread keeps its 16 points of the three 2^k sub-tiles, radix-3 step on registers.
 #pragma once
 #include <cuda.h>
@@ -149,7 +150,7 @@ struct TmaGeo {
     static constexpr int TILE = L * NB;            // points per tile
     static constexpr int NBOX = (L + 255) / 256;   // a TMA box dimension is at most 256
     static constexpr int LB = L / NBOX;
-    static constexpr bool PIN = V == V_LOSS || V == V_HEIGHT || V == V_GRAD;
+    static constexpr bool PIN = V == V_LOSS || V == V_HEIGHT || V == V_GRAD || V == V_LDOTHER || V == V_STOTHER;
     static constexpr bool FIELD_IN = V != V_HEIGHT;
     static constexpr bool FIELD_OUT = V != V_GRAD;
     static constexpr int FIELD_BYTES = TILE * 8;
@@ -176,6 +177,7 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
     extern __shared__ __align__(128) unsigned char tm_raw[];
     __shared__ uint64_t full[NST], done[NST];
     __shared__ double red[2][NCOMP / 32 > 0 ? NCOMP / 32 : 1];
+    __shared__ double red4[V == V_STOTHER ? 2 : 1][4][NCOMP / 32 > 0 ? NCOMP / 32 : 1]; // plane sums of the si-mse pass
 
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -196,7 +198,10 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
     // ================================================================ producer warp
     if (tid >= NCOMP) {
         if (tid != NCOMP) return;
-        const bool store_plane = V == V_GRAD || (V == V_LOSS && p.write_intensity);
+        // which fp32 plane tiles move: the run-time load / store op of the V_LDOTHER / V_STOTHER flavours decides
+        const bool store_plane = V == V_GRAD || (V == V_LOSS && p.write_intensity) ||
+                                 (V == V_STOTHER && (p.store_op == ST_C64_INTENSITY || p.write_intensity));
+        const bool load_plane = G::PIN && !(V == V_STOTHER && p.store_op != ST_C64_STATS);
         auto coords = [&](unsigned k, int* c0, int* c1, int* c3) {
             unsigned t = first + k * stride;
             *c0 = (int)((t % ncg) + (unsigned)p.cg0) * NB;
@@ -208,11 +213,11 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
             const int s = (int)(k % NST);
             int c0, c1, c3;
             coords(k, &c0, &c1, &c3);
-            tm_mbar_expect_tx(&full[s], (G::FIELD_IN ? G::FIELD_BYTES : 0) + G::PLANE_BYTES);
+            tm_mbar_expect_tx(&full[s], (G::FIELD_IN ? G::FIELD_BYTES : 0) + (load_plane ? G::PLANE_BYTES : 0));
 #pragma unroll
             for (int b = 0; b < G::NBOX; ++b) {
                 if (G::FIELD_IN) tm_load(fbuf(s) + b * G::LB * NB, &maps.field, &full[s], c0, c1, b * G::LB, c3);
-                if (G::PIN) tm_load(pbuf(s) + b * G::LB * NB, &maps.pin, &full[s], c0, c1, b * G::LB, c3);
+                if (load_plane) tm_load(pbuf(s) + b * G::LB * NB, &maps.pin, &full[s], c0, c1, b * G::LB, c3);
             }
         };
         for (unsigned k = 0; k < (unsigned)NST && k < n_my; ++k) load(k);
@@ -303,6 +308,17 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                     }
                 } else {
                     TL::template from_smem<0>(v, B, tt, col);
+                    if (V == V_LDOTHER) { // A1 on a stored field: g_u = 2 (dL/dI) u  /  Eq. (6): (c0 + cI |u|^2 + cT T) u
+                        const bool simse = p.load_op == LD_SEED_SIMSE;
+                        const float k0 = simse ? __ldg(p.coef) : 0.0f, k1 = simse ? __ldg(p.coef + 1) : 0.0f,
+                                    k2 = simse ? __ldg(p.coef + 2) : 2.0f;
+#pragma unroll
+                        for (int i = 0; i < P; ++i) {
+                            const float pl = Pl[(tt + i * T) * NB + col];
+                            const float g = fmaf(k1, v[i].x * v[i].x + v[i].y * v[i].y, fmaf(k2, pl, k0));
+                            v[i] = make_float2(g * v[i].x, g * v[i].y);
+                        }
+                    }
                 }
                 fwd_groups<TL, S, 0, NCOMP>(v, B, tt, col, tw);
             } else {
@@ -382,6 +398,42 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
                 }
             } else {
                 TL::template to_smem<0>(v, B, tt, col);
+                if (V == V_STOTHER) { // keep u; I = |u|^2 [and the plane sums <I,T>, <I,I>, sum I, <T,T> of Eq. (6)]
+                    const bool stats = p.store_op == ST_C64_STATS;
+                    double st0 = 0.0, st1 = 0.0, st2 = 0.0, st3 = 0.0;
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        float* tp = Pl + (tt + i * T) * NB + col;
+                        const float I = v[i].x * v[i].x + v[i].y * v[i].y;
+                        if (stats) {
+                            const float Tv = *tp;
+                            st0 += (double)I * (double)Tv;
+                            st1 += (double)I * (double)I;
+                            st2 += (double)I;
+                            st3 += (double)Tv * (double)Tv;
+                        }
+                        if (!stats || p.write_intensity) *tp = I;
+                    }
+                    if (stats) { // deterministic CTA reduction of the four sums
+#pragma unroll
+                        for (int d = 16; d > 0; d >>= 1) {
+                            st0 += __shfl_down_sync(0xffffffffu, st0, d);
+                            st1 += __shfl_down_sync(0xffffffffu, st1, d);
+                            st2 += __shfl_down_sync(0xffffffffu, st2, d);
+                            st3 += __shfl_down_sync(0xffffffffu, st3, d);
+                        }
+                        if ((tid & 31) == 0) {
+                            red4[k & 1][0][tid >> 5] = st0; red4[k & 1][1][tid >> 5] = st1;
+                            red4[k & 1][2][tid >> 5] = st2; red4[k & 1][3][tid >> 5] = st3;
+                        }
+                        cbar();
+                        if (tid < 4) {
+                            double r = 0.0;
+                            for (int w = 0; w < NCOMP / 32; ++w) r += red4[k & 1][tid][w];
+                            p.loss_scratch[4 * (p.tile0 + tile_id) + tid] = r;
+                        }
+                    }
+                }
             }
         } else {
             // ---- digits 3 * LP: a thread keeps its 16 points of all three LP-point sub-tiles (48 points; the CTA is alone
@@ -661,11 +713,12 @@ static cudaError_t launch_tma_one(const PassDesc& p, cudaStream_t stream)
     // the rest of a loaded tile with zeros and clips the stored one (needs the line to be the whole x axis: n_m = 1)
     const long long pslots = p.ap_nx > 0 ? p.L / 2 : 0, pso = p.ap_nx > 0 ? p.ap_nx : 0;
     if (p.ap_nx > 0 && (p.n_m != 1 || G::PIN == false)) return cudaErrorInvalidValue;
-    if (G::PIN) {
-        const float* src = V == V_LOSS ? p.plane_in : p.height;
+    if (G::PIN && !(V == V_STOTHER && p.store_op != ST_C64_STATS)) {
+        const float* src = (V == V_LOSS || V == V_LDOTHER || V == V_STOTHER) ? p.plane_in : p.height;
         if (!tma_make_map(&maps.pin, src, 4, p, NB, G::LB, pslots, pso)) return cudaErrorInvalidValue;
     }
-    if (V == V_GRAD || (V == V_LOSS && p.write_intensity)) {
+    if (V == V_GRAD || (V == V_LOSS && p.write_intensity) ||
+        (V == V_STOTHER && (p.store_op == ST_C64_INTENSITY || p.write_intensity))) {
         if (!tma_make_map(&maps.pout, p.plane_out, 4, p, NB, G::LB, pslots, pso)) return cudaErrorInvalidValue;
     }
     const int per_sm = (p.device >= 0 && p.device < 64) ? resident[p.device].load() : 1;
@@ -694,6 +747,10 @@ cudaError_t launch_tma(const PassDesc& p, int variant, int twb, cudaStream_t st)
             if (variant == V_LOSS) return launch_tma_one<L, NB, V_LOSS, TWB_LANE, NST>(p, st);
             if (variant == V_HEIGHT) return launch_tma_one<L, NB, V_HEIGHT, TWB_LANE, NST>(p, st);
             if (variant == V_GRAD) return launch_tma_one<L, NB, V_GRAD, TWB_LANE, NST>(p, st);
+            if (variant == V_LDOTHER && (p.load_op == LD_SEED || p.load_op == LD_SEED_SIMSE))
+                return launch_tma_one<L, NB, V_LDOTHER, TWB_LANE, NST>(p, st);
+            if (variant == V_STOTHER && (p.store_op == ST_C64_INTENSITY || p.store_op == ST_C64_STATS))
+                return launch_tma_one<L, NB, V_STOTHER, TWB_LANE, NST>(p, st);
         }
     }
     return kNotInstantiated;
