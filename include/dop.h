@@ -62,7 +62,8 @@ typedef enum {
     DOP_ERR_WORKSPACE = 3,        /* NULL workspace                                              */
     DOP_ERR_STATE = 4,            /* adj called before fwd                                       */
     DOP_ERR_ARCH = 5,             /* current device is not compute capability 10.x (sm_100)      */
-    DOP_ERR_CUDA = 6              /* a CUDA runtime call or launch failed (cudaGetLastError)     */
+    DOP_ERR_CUDA = 6,             /* a CUDA runtime call or launch failed (cudaGetLastError)     */
+    DOP_ERR_NOALLOC_LIMIT = 7     /* dop_prefilter_noalloc: ny * nx > DOP_NOALLOC_MAX_POINTS     */
 } dop_status;
 
 typedef enum {
@@ -220,6 +221,31 @@ dop_status dop_propagate_adj(dop_plan* plan, const void* d_height, const float* 
 dop_status dop_propagate_adj_adam(dop_plan* plan, float* d_layout, const float* d_dLdI, float* d_grad_height,
                                   float* d_m, float* d_v, const dop_adam* hp, void* d_workspace,
                                   void* cuda_stream);
+
+/*
+ * The Gaussian pre-filter F0 / A6 (the blur of the MTF model PAPER.md:184, standing in for G{l} of Eq. 5
+ * PAPER.md:114-122; F0) for callers that cannot allocate: code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc.  It is the stencil form of the pre-filter that dop_propagate_fwd /
+ * dop_propagate_adj run (rows into a scratch plane, columns out of it), except that the scratch plane is a static
+ * device array inside the library (DOP_NOALLOC_MAX_POINTS floats = 16 MiB, held by every GPU that loads the
+ * library until the process exits) instead of the caller's workspace, and that it needs no device tables of the
+ * plan.  The call reaches no cudaMalloc, cudaFree or allocating library routine, on its first use or later.
+ *   plan         a plan whose pre-filter runs as a stencil: prefilter_sigma_px in [2.05, 4], fp32 layout without
+ *                up-sampling, nx % 8 == 0, ny % 32 == 0, no tuning.no_stencil / force_generic; only its HOST side
+ *                is read (shape and taps), so it may be a plan that never ran, on any device.
+ *                Anything else -> DOP_ERR_INVALID_ARG.
+ *   d_in         [ny][nx] fp32 DEVICE (current device), read-only: h (F0) or dL/dh_eff (A6; the filter is even).
+ *   d_out        [ny][nx] fp32 DEVICE, overwritten; may be d_in itself, must not overlap it otherwise.
+ *   cuda_stream  cudaStream_t; the two kernels are enqueued on it, nothing is synchronised.
+ * Limit: ny * nx <= DOP_NOALLOC_MAX_POINTS, else DOP_ERR_NOALLOC_LIMIT (nothing is enqueued).
+ * Sharing: all calls on a device use the one array, which keeps the previous call's contents; none of it has to
+ * start at zero (the row kernel overwrites every element the column kernel reads), so nothing is cleared.  Calls
+ * that OVERLAP on the GPU -- two streams, or graph branches with no edge between them -- race on it; order them.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress) and loads the two kernels; make
+ * that call outside stream capture.  Errors: DOP_ERR_ARCH off sm_100, DOP_ERR_CUDA.
+ */
+#define DOP_NOALLOC_MAX_POINTS (4 * 1024 * 1024)
+dop_status dop_prefilter_noalloc(const dop_plan* plan, const float* d_in, float* d_out, void* cuda_stream);
 
 /* Frees the plan's host memory and device tables.  NULL -> DOP_ERR_INVALID_ARG. */
 dop_status dop_plan_destroy(dop_plan* plan);

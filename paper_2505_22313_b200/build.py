@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdop.so")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu", "blur.cu"]
+SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu", "blur.cu", "noalloc.cu"]
 # (column-type?, digit length) -- must match the DOP_DECL list in kernels_pow2.cu
 POW2_INST = [(1, L) for L in (16, 32, 64, 128, 256, 512)] + \
             [(0, L) for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192)]

@@ -658,6 +658,7 @@ const char* dop_status_string(dop_status s)
     case DOP_ERR_STATE: return "DOP_ERR_STATE: dop_propagate_adj needs a preceding dop_propagate_fwd";
     case DOP_ERR_ARCH: return "DOP_ERR_ARCH: device is not sm_100";
     case DOP_ERR_CUDA: return "DOP_ERR_CUDA: CUDA runtime error (see cudaGetLastError)";
+    case DOP_ERR_NOALLOC_LIMIT: return "DOP_ERR_NOALLOC_LIMIT: dop_prefilter_noalloc takes at most DOP_NOALLOC_MAX_POINTS = 4194304 points (its static scratch array)";
     }
     return "DOP_ERR_UNKNOWN";
 }

@@ -20,6 +20,8 @@ DOP_ERR_WORKSPACE = 3
 DOP_ERR_STATE = 4
 DOP_ERR_ARCH = 5
 DOP_ERR_CUDA = 6
+DOP_ERR_NOALLOC_LIMIT = 7
+DOP_NOALLOC_MAX_POINTS = 4 * 1024 * 1024
 DOP_LOSS_NONE = 0
 DOP_LOSS_L2 = 1
 DOP_LOSS_SIMSE = 2
@@ -92,6 +94,8 @@ def _load() -> C.CDLL:
     lib.dop_propagate_adj.restype = C.c_int
     lib.dop_propagate_adj_adam.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(dop_adam), vp, vp]
     lib.dop_propagate_adj_adam.restype = C.c_int
+    lib.dop_prefilter_noalloc.argtypes = [vp, vp, vp, vp]
+    lib.dop_prefilter_noalloc.restype = C.c_int
     lib.dop_plan_destroy.argtypes = [vp]
     lib.dop_plan_destroy.restype = C.c_int
     lib.dop_status_string.argtypes = [C.c_int]
@@ -110,7 +114,7 @@ def _load() -> C.CDLL:
 
 
 _lib = _load()
-EXPORTS = ("dop_plan_create", "dop_propagate_fwd", "dop_propagate_adj", "dop_propagate_adj_adam", "dop_plan_destroy",
+EXPORTS = ("dop_plan_create", "dop_propagate_fwd", "dop_propagate_adj", "dop_propagate_adj_adam", "dop_prefilter_noalloc", "dop_plan_destroy",
            "dop_status_string", "dop_plan_describe", "dop_plan_launch_count",
            "dop_plan_set_profiling", "dop_plan_get_pass_times", "dop_plan_pass_name")
 
@@ -183,6 +187,14 @@ def dop_propagate_adj_adam(plan, d_layout, d_dLdI, d_grad_height, d_m, d_v, lr0:
                                      None if d_workspace is None else d_workspace.data_ptr(), _stream(stream))
     if st != DOP_OK:
         raise DopError(st, "dop_propagate_adj_adam")
+
+
+def dop_prefilter_noalloc(plan, d_in, d_out, stream=None) -> None:
+    """The stencil pre-filter through the library's static scratch array (no allocation; include/dop.h)."""
+    st = _lib.dop_prefilter_noalloc(plan, _ptr(d_in, torch.float32, "d_in"), _ptr(d_out, torch.float32, "d_out"),
+                                    _stream(stream))
+    if st != DOP_OK:
+        raise DopError(st, "dop_prefilter_noalloc")
 
 
 def dop_plan_destroy(plan) -> None:
