@@ -116,6 +116,9 @@ typedef struct {
     int32_t tma_stages;     /* 1..8: tiles in flight per CTA of the TMA kernels (0 = per-pass default)          */
     int32_t no_stencil;     /* != 0: the Gaussian pre-filter always runs in its spectral form (ten FFT passes)  */
                             /*       instead of the separable spatial stencil used for 2 <= sigma <= 4 px (blur.cu) */
+    int32_t no_smooth;      /* != 0: plain passes of the 5-smooth digits 225, 625, 900, 2500 (the paper's 28 800 and     */
+                            /*       40 000 grids) through the generic kernel instead of the register-step kernels       */
+                            /*       (smooth.cu)                                                                         */
 } dop_tuning;
 
 typedef struct {

@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdop.so")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu", "blur.cu", "noalloc.cu"]
+SOURCES = ["api.cu", "plan.cu", "kernels_generic.cu", "kernels_pow2.cu", "blur.cu", "noalloc.cu", "smooth.cu"]
 # (column-type?, digit length) -- must match the DOP_DECL list in kernels_pow2.cu
 POW2_INST = [(1, L) for L in (16, 32, 64, 128, 256, 512)] + \
             [(0, L) for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192)]
@@ -26,7 +26,7 @@ POW2_X3 = (16, 32, 64, 128)  # digits 3 * LP
 TMA_INST = [(16, 32, 3), (32, 32, 3), (64, 32, 3), (64, 16, 3), (128, 32, 3), (128, 16, 3), (256, 32, 2), (256, 16, 3), (256, 16, 2), (512, 16, 2),
             (96, 32, 3), (192, 32, 3), (384, 32, 2)]
 CLUSTER_INST = [(4096, 2), (4096, 1), (2048, 4), (1024, 8)]  # (local transform length M, lines per CTA S): rows of 16 M
-HEADERS = ["dop_internal.h", "fft_regs.cuh", "pow2_impl.cuh", "cluster_row.cuh", "tma_col.cuh", os.path.join("..", "..", "include", "dop.h")]
+HEADERS = ["dop_internal.h", "bfly.cuh", "fft_regs.cuh", "pow2_impl.cuh", "cluster_row.cuh", "tma_col.cuh", os.path.join("..", "..", "include", "dop.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC",

@@ -12,12 +12,15 @@
 namespace dop {
 cudaError_t launch_tile_pass_generic(const PassDesc& p, cudaStream_t stream);
 cudaError_t launch_tile_pass_pow2(const PassDesc& p, cudaStream_t stream, bool* handled);
+cudaError_t launch_tile_pass_smooth(const PassDesc& p, cudaStream_t stream, bool* handled);
 
 cudaError_t launch_tile_pass(const PassDesc& p, cudaStream_t stream)
 {
     {
         bool handled = false;
         cudaError_t e = launch_tile_pass_pow2(p, stream, &handled);
+        if (handled) return e;
+        e = launch_tile_pass_smooth(p, stream, &handled);
         if (handled) return e;
     }
     return launch_tile_pass_generic(p, stream);

@@ -119,6 +119,7 @@ struct PassDesc {
                           // has rows of grid_nx points; plane accesses outside the aperture are masked (ap_nx = 0: no padding)
     const int* hpair;     // (x) H pass on mirrored tile pairs (tma_hpair_kernel): n_hpair items (o_A, o_B | -1), or nullptr
     int n_hpair;
+    int smooth;           // 1: plain pass of a 5-smooth digit on the register-step kernels (smooth.cu); nl / threads / smem are theirs
     int tma;              // > 0: TMA column kernel (tma_col.cuh) with this many tiles in flight per CTA; nl = its bundle width
 };
 
@@ -131,6 +132,10 @@ bool cluster_instantiated(long long L1, int lines);
 bool tma_instantiated(long long L, int nb, int nst);
 int pow2_lines(long long L, bool col_type, bool plain = false, int nb_override = 0);
 std::vector<float2> pow2_group_twiddles(long long L);
+// plain passes of the 5-smooth digits 225, 625, 900, 2500 (smooth.cu)
+std::vector<int> smooth_radix(long long L);
+bool smooth_supported(long long L, bool col_type);
+void smooth_geometry(long long L, bool col_type, int* nl, int* threads, int* smem_bytes);
 cudaError_t launch_loss_reduce(const double* scratch, long long n, double inv_n, double* d_loss,
                                cudaStream_t stream);
 // DOP_LOSS_SIMSE: plane sums -> scale s, loss, seed coefficients per wavelength (kernels_generic.cu)
@@ -159,6 +164,7 @@ struct Digit {
     std::vector<float2> twb;      // W_{L st}^p, p < L st
     size_t twb_off = 0;           // byte offset into the device arena
     bool fast = false;            // handled by the register-blocked pow2 kernels
+    bool smooth = false;          // its plain passes run on the register-step kernels of smooth.cu
     std::vector<float2> twg;      // their group twiddles
     size_t twg_off = 0;
     std::vector<float2> twb2;     // boundary twiddles in the pow2 kernels' layout (fast digits with has_twb)

@@ -37,7 +37,8 @@ static bool is_23_smooth(long long n)
 // radix steps for one digit: odd primes > 3 first (largest first), then 3s, then 4s, then one 2 if needed
 static std::vector<int> radix_steps(long long L)
 {
-    std::vector<int> r;
+    std::vector<int> r = smooth_radix(L); // 225, 625, 900, 2500: the order the register-step kernels run (smooth.cu)
+    if (!r.empty()) return r;
     for (long long q = kMaxPrime; q >= 5; --q)
         while (L % q == 0 && prime_factors(q).size() == 1) { r.push_back((int)q); L /= q; }
     while (L % 3 == 0) { r.push_back(3); L /= 3; }
@@ -79,7 +80,7 @@ static std::vector<float2> twiddle_table(long long n)
 // <= lmax_last, as balanced as possible.  A forced decomposition (dop_tuning) overrides; it must
 // multiply to N and respect the same limits.
 static bool split_digits(long long N, long long lmax_first, long long lmax_last, int n_forced,
-                         const int64_t* forced, std::vector<long long>* out, bool last_is_row)
+                         const int64_t* forced, std::vector<long long>* out, bool last_is_row, bool tu_no_smooth)
 {
     out->clear();
     if (n_forced > 0) {
@@ -123,6 +124,7 @@ static bool split_digits(long long N, long long lmax_first, long long lmax_last,
             // (fused x passes stage their fp32 planes by TMA: the line count N / dgt must be a multiple of 4)
             const bool planes_ok = !(last_is_row && first && !last) || (N / dgt) % 4 == 0;
             if (pow2_supported(dgt, col) && !(fused && dgt % 3 == 0) && planes_ok) return 1.0;
+            if (!fused && !tu_no_smooth && smooth_supported(dgt, col)) return 1.5; // register-step kernels (smooth.cu)
             const std::vector<long long> f = prime_factors(dgt);
             return (fused ? 6.0 : 4.0) + (f.back() > 7 ? (double)f.back() / 4.0 : 0.0);
         };
@@ -218,8 +220,10 @@ static bool build_axis(dop_plan* p, int a, long long N, const std::vector<long l
         // kernels, where the TMA unit itself masks the planes to the aperture (resolve() sends anything else to the generic kernel)
         const bool pad_tma = Ls.size() == 2 && (d.L & (d.L - 1)) == 0 && d.L >= 16 && !tu_no_tma && !p->force_generic;
         if (p->ap_nx > 0 && a == 0 && j == 0 && !pad_tma) d.fast = false;
+        // 5-smooth digits with register-step kernels for their plain passes (smooth.cu)
+        d.smooth = !p->force_generic && !p->tune.no_smooth && !d.fast && smooth_supported(d.L, col_type);
         if (d.fast) d.twg = pow2_group_twiddles(d.L);
-        if (d.fast && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
+        if ((d.fast || (d.smooth && col_type)) && d.has_twb) { // W_{N_j}^{r pi[slot]}: y digits [r][slot], x digits [slot][r]
             const long long Nj = d.L * d.st;
             d.twb2.resize((size_t)Nj);
             for (long long r = 0; r < d.st; ++r)
@@ -419,6 +423,12 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
     }
     tile_geometry(p, t.axis, t.digit, d);
     const Digit& g = p->ax[t.axis].dig[(size_t)t.digit];
+    if (g.smooth && t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_C64 && t.store_op == ST_C64) {
+        smooth_geometry(g.L, d->col_type != 0, &d->nl, &d->threads, &d->smem_bytes);
+        d->n_cgroups = (d->NC + d->nl - 1) / d->nl;
+        d->smooth = 1;
+        return;
+    }
     if (!g.fast || !d->col_type) return;
     // Column passes the TMA kernels implement (tma_col.cuh) run there: bundle width and pipeline depth per
     // digit length and variant (measured, profiles/r02_tma_col.md), dop_tuning.tma_nb / tma_stages override.
@@ -544,8 +554,8 @@ dop_status build_plan(dop_plan* p)
                               (tu.cluster_force || d.nx == 16384);
     if (want_cluster && tu.n_xdigits == 0) {
         lx = {16, d.nx / 16}; // rows of 16 M points: one thread-block-cluster pass per transform pair
-    } else if (!split_digits(d.nx, 512, 8192, tu.n_xdigits, tu.xdigits, &lx, true)) return DOP_ERR_UNSUPPORTED_SIZE;
-    if (!split_digits(d.ny, 512, 512, tu.n_ydigits, tu.ydigits, &ly, false)) return DOP_ERR_UNSUPPORTED_SIZE;
+    } else if (!split_digits(d.nx, 512, 8192, tu.n_xdigits, tu.xdigits, &lx, true, tu.no_smooth != 0)) return DOP_ERR_UNSUPPORTED_SIZE;
+    if (!split_digits(d.ny, 512, 512, tu.n_ydigits, tu.ydigits, &ly, false, tu.no_smooth != 0)) return DOP_ERR_UNSUPPORTED_SIZE;
     if (!build_axis(p, 0, d.nx, lx) || !build_axis(p, 1, d.ny, ly)) return DOP_ERR_UNSUPPORTED_SIZE;
     p->x_cluster = want_cluster && lx.size() == 2 && cluster_supported(lx[0], lx[1]) && p->ax[0].dig[0].fast &&
                    p->ax[0].dig[1].fast;
@@ -668,7 +678,7 @@ std::string describe_plan(const dop_plan* p)
                 os << tag << " x0+x1 L=16x" << g.L << " tile=" << g.nl << "x" << g.L << " row cluster=" << g.n_cgroups;
             else
                 os << tag << " " << (t.axis == 0 ? "x" : "y") << t.digit << " L=" << g.L << " tile=" << g.nl << "x" << g.L
-                   << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? (g.tma ? " tma" : " pow2") : " generic");
+                   << (g.col_type ? " col" : " row") << (p->ax[t.axis].dig[(size_t)t.digit].fast ? (g.tma ? " tma" : " pow2") : (g.smooth ? " smooth" : " generic"));
             if (g.tma) os << " stages=" << g.tma;
             os << " ctas=" << g.n_cgroups * g.n_m * g.n_o
                << " smem=" << g.smem_bytes << " B/pt=" << t.bytes_per_point << " [" << t.name << "]\n";

@@ -38,7 +38,7 @@ class dop_tuning(C.Structure):
         ("force_generic", C.c_int32), ("col_nb", C.c_int32), ("prefetch_waves", C.c_int32), ("slab_mb", C.c_int32),
         ("slab_streams", C.c_int32), ("h_float", C.c_int32), ("tile_pts", C.c_int32), ("no_cluster", C.c_int32),
         ("no_mirror", C.c_int32), ("cluster_dsmem", C.c_int32), ("cluster_lines", C.c_int32), ("cluster_force", C.c_int32),
-        ("no_tma", C.c_int32), ("tma_nb", C.c_int32), ("tma_stages", C.c_int32), ("no_stencil", C.c_int32),
+        ("no_tma", C.c_int32), ("tma_nb", C.c_int32), ("tma_stages", C.c_int32), ("no_stencil", C.c_int32), ("no_smooth", C.c_int32),
     ]
 
 

@@ -244,18 +244,21 @@ def test_loss_scratch_matches_the_launched_loss_pass():
 
 @pytest.mark.parametrize("ny,nx,expect", [
     (3600, 3600, ["x-digits: 3600(", "radix=5.5.3.3.4.4", "y1 L=16 tile=32x16 col tma"]),                  # PAPER.md:274 Table 2
-    (28800, 28800, ["x-digits: 32(st=900,radix=4.4.2) 900(st=1,radix=5.5.3.3.4)", "y-digits: 225(st=128,radix=5.5.3.3) 128(",
-                    "x0 L=32 tile=32x32 col tma", "y1 L=128 tile=16x128 col tma", "x1 L=900 tile=4x900 row generic"]),
-    (40000, 40000, ["x-digits: 16(st=2500,radix=4.4) 2500(st=1,radix=5.5.5.5.4)", "y-digits: 625(st=64,radix=5.5.5.5) 64(",
-                    "x0 L=16 tile=32x16 col tma", "y1 L=64 tile=16x64 col tma"]),
+    (28800, 28800, ["x-digits: 32(st=900,radix=4.4.2) 900(st=1,radix=5.3.2.5.3.2)", "y-digits: 225(st=128,radix=5.3.5.3) 128(",
+                    "x0 L=32 tile=32x32 col tma", "y1 L=128 tile=16x128 col tma", "x1 L=900 tile=8x900 row smooth",
+                    "y0 L=225 tile=32x225 col smooth"]),
+    (40000, 40000, ["x-digits: 16(st=2500,radix=4.4) 2500(st=1,radix=5.5.2.5.5.2)", "y-digits: 625(st=64,radix=5.5.5.5) 64(",
+                    "x0 L=16 tile=32x16 col tma", "y1 L=64 tile=16x64 col tma", "x1 L=2500 tile=4x2500 row smooth",
+                    "y0 L=625 tile=16x625 col smooth"]),
     (128640, 85760, ["x-digits: 64(st=1340,radix=4.4.4) 1340(st=1,radix=67.5.4)", "y-digits: 384(st=335", "335(st=1,radix=67.5)",
                      "x0 L=64 tile=16x64 col tma", "y0 L=384 tile=32x384 col tma"]),
 ])
 def test_the_papers_own_grid_sizes_plan(ny, nx, expect):
     """the grids of PAPER.md:270-280 (Table 2) factor into digits with prime factors 5 and 67; the
     plan puts the fused passes (first x digit, last y digit) on power-of-two digits, i.e. on the specialised
-    kernels -- a ragged last column tile (225 or 335 lines) is clipped by the TMA unit -- and gives the odd primes
-    to the generic kernel's direct butterflies.  128 640 x 85 760 (the paper's 16-GPU grid) fits one B200 in place: field 82.2 GiB."""
+    kernels -- a ragged last column tile (225 or 335 lines) is clipped by the TMA unit --, runs the plain passes of the
+    5-smooth digits 225 / 625 / 900 / 2500 on the register-step kernels (smooth.cu) and gives the prime 67 to the generic
+    kernel's direct butterflies.  128 640 x 85 760 (the paper's 16-GPU grid) fits one B200 in place: field 82.2 GiB."""
     h, ws = dop.dop_plan_create(ny, nx, 0.5e-6, (520.6e-9,), (1.5,), 0.06)
     text = dop.dop_plan_describe(h)
     dop.dop_plan_destroy(h)

@@ -224,6 +224,44 @@ def test_H_on_mirrored_tile_pairs_against_the_oracle(ny, yd, nx, xd):
     assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
 
 
+@pytest.mark.parametrize("ny,yd,nx,xd", [
+    (450, "225,2", 1800, "2,900"),        # 225 as a y digit (ragged last column tile), 900 as the row-type last x digit
+    (10000, "", 72, ""),                  # 625 as a y digit (the planner's 625 . 16; ragged last column tile)
+    (7, "", 5000, "2,2500"),              # 2500 as the last x digit (ragged last row tile)
+    (64, "64", 900, "4,225"),             # 225 as the last x digit
+    (64, "64", 1250, "2,625"),            # 625 as the last x digit (odd line length: 8-byte staging)
+    (900, "2,225,2", 7200, "2,225,16"),   # 225 as a middle digit of both axes (x: lines = 16 < tile width, per-line twiddles)
+    (3600, "225,16", 14400, "16,900"),    # the digit pairs the planner picks for the paper's 28 800 grid, on the TMA kernels
+])
+def test_smooth_digit_passes_against_the_oracle(ny, yd, nx, xd):
+    """Plain passes of the 5-smooth digits 225, 625, 900, 2500 (the paper's 28 800 and 40 000 grids)
+    on the register-step kernels (smooth.cu), column- and row-type, forward and inverse, against the oracle and
+    against the generic kernel running the same schedule (dop_tuning.no_smooth)."""
+    cfg = synth.CONFIGS["C4"].scaled(ny, nx)
+    h, T = synth.make_height(cfg, DEV), synth.make_target(cfg, DEV)
+    tun = dict(ydigits=digits(yd) if yd else (), xdigits=digits(xd) if xd else ())
+    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, tuning=dop.make_tuning(**tun))
+    text = plan.describe()
+    plan.close()
+    plain = [l for l in text.splitlines() if l.endswith(("[x-fwd]", "[x-inv]", "[y-fwd]", "[y-inv]"))]
+    for L in (225, 625, 900, 2500):
+        for l in plain:
+            if f" L={L} " in l:
+                assert " smooth " in l, text
+    assert any(" smooth " in l for l in plain), text
+    plan = dop.Plan(ny, nx, cfg.pitch, cfg.lambdas, cfg.n_refr, cfg.z, tuning=dop.make_tuning(no_smooth=1, **tun))
+    assert " smooth " not in plan.describe()
+    plan.close()
+    I, L, g = run_l2(cfg, h, T, tuning=dop.make_tuning(**tun))
+    Ir, Lr, gr = oracle_l2(cfg, h, T)
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+    I0, L0, g0 = run_l2(cfg, h, T, tuning=dop.make_tuning(no_smooth=1, **tun))
+    check(I, I0, "intensity against the generic kernel")
+    check(g, g0, "dL/dh against the generic kernel")
+
+
 @pytest.mark.parametrize("ny,nx", [(8, 16384), (6, 32768), (4, 65536), (96, 65536)])
 def test_cluster_row_passes_against_the_oracle(ny, nx):
     """Rows of 16 M points (M = 1024, 2048, 4096) run their two x digit passes as ONE thread-block-cluster
