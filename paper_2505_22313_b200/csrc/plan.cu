@@ -441,10 +441,11 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
         const bool lossp = t.mid_op == MID_LOSS && t.fft1_dir < 0 && t.fft2_dir > 0 && t.load_op == LD_C64 && t.store_op == ST_C64;
         const bool heightp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_HEIGHT && t.store_op == ST_C64 && plain_layout;
         const bool gradp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_C64 && t.store_op == ST_GRAD && plain_layout;
-        // (h -> exp(i Phi) -> DFT: measured SLOWER through TMA than through the LDG/STG kernel on the bench inputs -- C4
-        // 18.6 against 13.5 ms, C5 27.9 against 20.5 -- so it goes there only when that kernel cannot run the pass:
-        // a line count that is not a multiple of 16)
-        const bool heightp_tma = heightp && (d->NC % 16 != 0 || p->ap_nx > 0); // (pad = 2: only the TMA kernel masks)
+        // (h -> exp(i Phi) -> DFT through TMA: 16-column tiles measured SLOWER than the LDG/STG kernel -- C4 14.6 against
+        // 13.7 ms, C5 22.0 against 21.0 -- and 32-column tiles of 256 slots faster -- C4 12.9, C5 19.7; so digits of 256
+        // go there, and otherwise only what that kernel cannot run: a line count that is not a multiple of 16, pad = 2)
+        const bool height_wide = heightp && g.L == 256 && d->NC % 32 == 0 && p->ap_nx == 0;
+        const bool heightp_tma = heightp && (height_wide || d->NC % 16 != 0 || p->ap_nx > 0); // (pad = 2: only the TMA kernel masks)
         // the split loss flavours: IDFT -> u, |u|^2 [, plane sums]  and  seed from u and dL/dI (or T) -> DFT
         const bool statp = t.mid_op == MID_NONE && t.fft2_dir == 0 && t.load_op == LD_C64 &&
                            (t.store_op == ST_C64_INTENSITY || t.store_op == ST_C64_STATS) && t.axis == 0;
@@ -460,7 +461,7 @@ static void pass_geometry_full(const dop_plan* p, const PassTmpl& t, PassDesc* d
             // with 32-column tiles, the register-heavy fused variants want 16 columns (two CTAs per SM)
             int nb = 32, nst = g.L <= 128 ? 3 : 2;
             if (sandwich || lossp || statp || seedp) { nb = 16; nst = 3; }
-            if (heightp_tma) { nb = 16; nst = g.L == 256 ? 2 : 3; }
+            if (heightp_tma) { nb = height_wide ? 32 : 16; nst = g.L == 256 ? 2 : 3; }
             if (g.L == 512) { nb = 16; nst = 2; }
             if (x3) { nb = 32; nst = g.L == 384 ? 2 : 3; }
             if (p->tma_nb) nb = p->tma_nb;

@@ -150,16 +150,14 @@ __device__ __forceinline__ void field_st(float2* p, float2 v)
     else *p = v;
 }
 
-// (cos 2 pi f, sin 2 pi f) for |f| < 2^20 turns: quadrant q = round(4f) mod 4 by the magic-number trick
-// (no F2I / FRND), residue |r| <= 1/8 turn, Taylor polynomials in r^2 (truncation 2e-9 / 2.4e-8),
-// then the quadrant rotation by selects and sign flips.  ~23 instructions against ~30 for the
-// library sincospif, which also has to handle arbitrary arguments.
-__device__ __forceinline__ void sincos_turn(float f, float* sn, float* cs)
+// (cos 2 pi f, sin 2 pi f) for |f| < 2^20 turns, polynomial form: quadrant q = round(4f) mod 4 by the magic-number
+// trick (no F2I / FRND), residue |r| <= 1/8 turn, Taylor polynomials in r^2 (truncation 2e-9 / 2.4e-8), then the
+// quadrant rotation by selects and sign flips.  ~23 instructions against ~30 for the library sincospif, which also
+// has to handle arbitrary arguments.  Used for the phase of H (apply_h; sincos_fixed / h_fixed_nb carry the same
+// polynomials): there the hardware sine / cosine measured no gain (three MUFU operations per H value on the
+// 16-lane pipe cost what the polynomial's FMAs do: C4 (x) H 17.0 -> 17.5-18.4 ms).
+__device__ __forceinline__ void sincos_turn_poly(float f, float* sn, float* cs)
 {
-#ifdef DOP_LIB_SINCOS
-    sincospif(2.0f * f, sn, cs);
-    return;
-#endif
     const float MAGIC = 12582912.0f;                 // 1.5 * 2^23
     const float t = fmaf(f, 4.0f, MAGIC);            // low mantissa bits = round(4 f) (two's complement)
     const int q = __float_as_int(t);
@@ -179,6 +177,27 @@ __device__ __forceinline__ void sincos_turn(float f, float* sn, float* cs)
     const float co = odd ? s : c, so = odd ? c : s;
     *cs = __int_as_float(__float_as_int(co) ^ (((q + 1) & 2) << 30));
     *sn = __int_as_float(__float_as_int(so) ^ ((q & 2) << 30));
+}
+// u0 = exp(i Phi) (F2, and its recomputation in A5): the residue r = f - rint(f) by the magic-number trick (exact),
+// then the hardware sine / cosine (MUFU.SIN / MUFU.COS behind sin.approx / cos.approx; measured on B200 over 2^26
+// arguments: max error 3.4e-7, rms 1.2e-7, including the rounding of 2 pi r) -- 8 instructions against 23, in
+// passes that are bound by instruction issue (C5 dL/dh pass 20.9 -> 18.7 ms, h -> exp(i Phi) 22.2 -> 21.2 ms).
+// -DDOP_POLY_SINCOS keeps the polynomial form.
+__device__ __forceinline__ void sincos_turn(float f, float* sn, float* cs)
+{
+#ifdef DOP_LIB_SINCOS
+    sincospif(2.0f * f, sn, cs);
+    return;
+#endif
+#ifndef DOP_POLY_SINCOS
+    const float RND = 12582912.0f;                   // 1.5 * 2^23: (f + RND) - RND = rint(f)
+    const float r = f - ((f + RND) - RND);           // exact (Sterbenz), |r| <= 1/2 turn
+    const float x = r * 6.283185307179586f;
+    *sn = __sinf(x);
+    *cs = __cosf(x);
+#else
+    sincos_turn_poly(f, sn, cs);
+#endif
 }
 // Any moderate argument in turns (|ph| < 2^20) needs no separate integer reduction: round(4 ph) mod 4
 // is the quadrant whatever the integer part, and ph - round(4 ph)/4 is exact (Sterbenz).
@@ -201,7 +220,7 @@ __device__ __forceinline__ float2 apply_h(float2 v, double c_minus_fx2, double f
         const double RND = 6755399441055744.0;                    // 1.5 * 2^52: (x + RND) - RND = rint(x)
         const float f = (float)(turns - ((turns + RND) - RND));   // fractional turn, |f| <= 0.5
         float sn, cs;
-        sincos_turn(f, &sn, &cs);
+        sincos_turn_poly(f, &sn, &cs);
         const float2 h = make_float2(cs * scale, (conj ? -sn : sn) * scale);
         return fx::cmul(v, h);
     }
@@ -278,6 +297,7 @@ __device__ __forceinline__ float2 h_fixed_nb(double c_minus_fx2, double fy2, dou
     double s = a * y;
     s = fma(fma(-s, s, a), 0.5 * y, s);
     const unsigned ph = (unsigned)__double2loint(fma(s, z32, 6755399441055744.0));
+    const bool prop = a >= 0.0; // evanescent bins are zeroed
     const unsigned t = ph + 0x20000000u;
     const int q = (int)(t >> 30);
     const int ri = (int)(t & 0x3FFFFFFFu) - 0x20000000;
@@ -295,7 +315,6 @@ __device__ __forceinline__ float2 h_fixed_nb(double c_minus_fx2, double fy2, dou
     const float cs0 = fmaf(cp, r2, hk.c[0]);
     const bool odd = (q & 1) != 0;
     const float co = odd ? sn0 : cs0, so = odd ? cs0 : sn0;
-    const bool prop = a >= 0.0; // evanescent bins are zeroed
     const float hx = prop ? __int_as_float(__float_as_int(co) ^ (((q + 1) & 2) << 30)) : 0.0f;
     const float hy = prop ? __int_as_float(__float_as_int(so) ^ ((q & 2) << 30)) : 0.0f;
     return make_float2(hx, hy);

@@ -150,10 +150,11 @@ def test_launch_count_follows_the_slab_schedule():
 @pytest.mark.parametrize("ny,nx,yd,xd,tun,expect", [
     (65536, 32, "256,256", "32", {}, ["y0 L=256 tile=32x256 col tma stages=2", "y1 L=256 tile=16x256 col tma stages=3"]),
     (65536, 32, "256,256", "32", {"no_tma": 1}, ["y0 L=256 tile=32x256 col pow2", "y1 L=256 tile=16x256 col pow2"]),
-    (16, 131072, "16", "256,512", {}, ["x0 L=256 tile=16x256 col pow2 ctas=512 smem=32768 B/pt=12",
+    (16, 131072, "16", "256,512", {}, ["x0 L=256 tile=32x256 col tma stages=2 ctas=256 smem=196608 B/pt=12",
                                       "x0 L=256 tile=16x256 col tma stages=3 ctas=512 smem=147456 B/pt=20",
                                       "x0 L=256 tile=32x256 col tma stages=2 ctas=256 smem=196608 B/pt=16 [x-inv,grad]",
                                       "x1 L=512 tile=8x512 row pow2"]),
+    (16, 131072, "16", "256,512", {"no_tma": 1}, ["x0 L=256 tile=16x256 col pow2 ctas=512 smem=32768 B/pt=12"]),
     (6144, 128, "384,16", "128", {}, ["y0 L=384 tile=32x384 col tma stages=2", "x0 L=128 tile=32x128 row pow2"]),
     (6144, 128, "384,16", "128", {"no_tma": 1}, ["y0 L=384 tile=32x384 col pow2"]),
     (64, 8192, "64", "8192", {}, ["x0 L=8192 tile=1x8192 row pow2", "y0 L=64 tile=16x64 col tma stages=3"]),
