@@ -215,8 +215,8 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
     }
 
     // ---- middle op (natural layout)
+    __shared__ double red[kClThreads / 32]; // V_LOSS: per-warp partial sums of the tile's loss
     if (V == V_LOSS) {
-        __shared__ double red[kClThreads / 32];
         double acc = 0.0;
 #pragma unroll
         for (int c = 0; c < P; ++c) {
@@ -230,13 +230,7 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
         }
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, d);
-        if (lane == 0) red[tid >> 5] = acc;
-        __syncthreads();
-        if (tid == 0) {
-            double r = 0.0;
-            for (int w = 0; w < kClThreads / 32; ++w) r += red[w];
-            p.loss_scratch[p.tile0 + blockIdx.x] = r;
-        }
+        if (lane == 0) red[tid >> 5] = acc; // (summed by thread 0 after the cluster barriers of the exchange below)
     }
 
     if (LAST > 0) {
@@ -259,6 +253,11 @@ cluster_row_kernel(const __grid_constant__ PassDesc p)
         }
         TL::template forward<0, true>(v, s, tt, soff, tw);
         store_lines();
+        if (V == V_LOSS && tid == 0) { // deterministic: warp order; off the path of the other warps
+            double r = 0.0;
+            for (int w = 0; w < kClThreads / 32; ++w) r += red[w];
+            p.loss_scratch[p.tile0 + blockIdx.x] = r;
+        }
     } else {
         // ---- natural-layout store (+ epilogue op)
         double st0 = 0.0, st1 = 0.0, st2 = 0.0, st3 = 0.0; // ST_C64_STATS: <I,T>, <I,I>, sum I, <T,T>

@@ -456,6 +456,9 @@ pow2_kernel(const __grid_constant__ PassDesc p)
         for (int i = 0; i < P; i += (RL >= 16 ? 16 : RL)) asm volatile("prefetch.global.L1 [%0];" ::"l"(fyp + DOP_KL(i)));
     }
 
+    __shared__ double red[32];                                     // V_LOSS: per-warp partial sums
+    constexpr int NW = (tile_threads(L, COL, NB) + 31) / 32;
+    constexpr bool LOSS_DEFER = S::NG > 1 && !TL::template local_exchange<0, 1>();
     float2 v[P];
     // ---- load (+ prologue op, + conj boundary twiddle before an inverse DFT)
     if (DIR1 > 0) {
@@ -560,7 +563,6 @@ pow2_kernel(const __grid_constant__ PassDesc p)
             v[i] = make_float2(v[i].x * g, v[i].y * g);
         }
     } else if (V == V_LOSS) { // registers hold spatial points in the first group's layout
-        __shared__ double red[32];
         double acc = 0.0;
         long long off = b0;
 #pragma unroll
@@ -579,17 +581,25 @@ pow2_kernel(const __grid_constant__ PassDesc p)
 #pragma unroll
         for (int d = SW / 2; d > 0; d >>= 1) acc += __shfl_down_sync(SMASK, acc, d, SW);
         if ((tid & 31) == 0) red[tid >> 5] = acc;
-        __syncthreads();
-        if (tid == 0) {
-            double r = 0.0;
-            constexpr int NW = (tile_threads(L, COL, NB) + 31) / 32;
-            for (int w = 0; w < NW; ++w) r += red[w];
-            p.loss_scratch[p.tile0 + blockIdx.x] = r;
+        // The warp sums are added up by thread 0 after the forward DFT when its first exchange is CTA-wide (a barrier
+        // between these writes and that read), so that no warp waits for the serial sum; else behind a barrier here.
+        if (!LOSS_DEFER) {
+            __syncthreads();
+            if (tid == 0) {
+                double r = 0.0;
+                for (int w = 0; w < NW; ++w) r += red[w];
+                p.loss_scratch[p.tile0 + blockIdx.x] = r;
+            }
         }
     }
 
     if (DIR2 > 0) TL::template forward<0, COL>(v, s, tt, soff, tw);
     else if (DIR2 < 0) TL::template inverse<GL, COL>(v, s, tt, soff, tw);
+    if (V == V_LOSS && LOSS_DEFER && tid == 0) {
+        double r = 0.0;
+        for (int w = 0; w < NW; ++w) r += red[w];
+        p.loss_scratch[p.tile0 + blockIdx.x] = r;
+    }
 
     // ---- store (+ boundary twiddle after a forward DFT, + epilogue op)
     if (LAST > 0) {

@@ -369,15 +369,20 @@ tma_col_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ TmaMa
 #pragma unroll
                 for (int d = 16; d > 0; d >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, d);
                 if ((tid & 31) == 0) red[k & 1][tid >> 5] = acc;
-                cbar();
-                if (tid == 0) {
-                    double r = 0.0;
-                    for (int w = 0; w < NCOMP / 32; ++w) r += red[k & 1][w];
-                    p.loss_scratch[p.tile0 + tile_id] = r;
-                }
+                // The warp sums are added up (warp order: deterministic) by thread 0 AFTER the forward DFT, whose first
+                // exchange is the barrier between these writes and that read -- red[] is double-buffered, the tile after
+                // next is the first to write this half again.  With a barrier of its own here and the serial sum right
+                // behind it, every warp waited for thread 0 at the DFT's exchange: C5 loss pass 34.3 -> 30.4 ms, C4
+                // 27.8 -> 23.1.  (Summing in the producer thread instead measured no gain at C4: 27.3.)
+                if constexpr (S::NG == 1) cbar(); // (a single-group digit has no exchange)
             }
             if (DIR2 > 0) fwd_groups<TL, S, 0, NCOMP>(v, B, tt, col, tw);
             else if (DIR2 < 0) inv_groups<TL, S, GL, NCOMP>(v, B, tt, col, tw);
+            if (V == V_LOSS && tid == 0) { // (serial on purpose: a shuffle tree over warp 0 here measured C4 21.9 -> 28.1 ms)
+                double r = 0.0;
+                for (int w = 0; w < NCOMP / 32; ++w) r += red[k & 1][w];
+                p.loss_scratch[p.tile0 + tile_id] = r;
+            }
             // ---- store (+ boundary twiddle after a forward DFT, + epilogue)
             if (LAST > 0) {
                 if (TWB == TWB_LANE) {
@@ -603,7 +608,9 @@ tma_hpair_kernel(const __grid_constant__ PassDesc p, const __grid_constant__ Tma
         for (int i = 0; i < P; i += RL) asm volatile("prefetch.global.L1 [%0];" ::"l"(fyp + DOP_KL(i)));
         float2 h[P];
         float2 v[P];
-        // ---- tile A: H evaluated
+        // ---- tile A: H evaluated (after the DFT: evaluating it before the wait for the tile, where a tile still in
+        //      flight would hide it, measured slower -- C5 25.8 -> 27.7 ms, C4 17.1 -> 18.1: 32 more live registers
+        //      through the forward DFT)
         {
             const unsigned s = j % NST;
             float2* B = fbuf(s);
