@@ -107,6 +107,28 @@ def test_fused_l2_loss_path(ny, nx):
     assert L2 == L and np.array_equal(g2, g)
 
 
+@pytest.mark.parametrize("ny,nx,tun", [(256, 1024, {}),                      # row kernel (one x digit)
+                                       (64, 8192, {"xdigits": (256, 32)}),   # h -> exp(i Phi) and dL/dh on the TMA kernels
+                                       (64, 8192, {"xdigits": (256, 32), "no_tma": 1}),
+                                       (64, 16384, {}),                      # thread-block-cluster row pass
+                                       (35, 55, {})])                        # generic kernel
+def test_exp_i_phi_over_several_turns_of_either_sign(ny, nx, tun):
+    """F1/F2 and A5 on heights between -4 and +4 turns of phase (the configurations stay within 0..1.2 turns): the
+    exact residue Phi/2pi - rint(Phi/2pi) and the hardware sine / cosine behind it (reading 9) in every kernel
+    family, against the oracle's fp64 exp(i Phi)."""
+    cfg = synth.CONFIGS["C2"].scaled(ny, nx)
+    lam, n = cfg.lambdas[1], cfg.n_refr[1]
+    turn = lam / (n - 1.0)                                       # height of one turn of phase
+    h = ((synth.uniform_plane(91, 3, ny, nx, DEV).view(ny, nx) - 0.5) * (8.0 * turn)).contiguous()
+    T = synth.make_target(cfg, DEV)
+    tuning = dop.make_tuning(**tun) if tun else None
+    I, L, g = run_l2(cfg, h, T, lambdas=(lam,), n_refr=(n,), tuning=tuning)
+    Ir, Lr, gr = oracle_l2(cfg, h, T, lambdas=(lam,), n_refr=(n,))
+    check(I, Ir, "intensity")
+    check(g, gr, "dL/dh")
+    assert abs(L - Lr) <= TOL_LOSS * abs(Lr)
+
+
 @pytest.mark.parametrize("ny,nx,sigma,no_stencil", [(48, 64, 3.0, 0), (384, 512, 3.0, 0), (384, 512, 3.0, 1), (1024, 1536, 3.0, 0),
                                                     (1024, 1536, 3.0, 1), (256, 640, 0.7, 0), (256, 640, 2.1, 0), (512, 512, 4.0, 0), (512, 512, 5.5, 0)])
 def test_prefilter_path(ny, nx, sigma, no_stencil):
